@@ -1,0 +1,253 @@
+"""Pins of the oracle's rate fits and chemistry operator Phi (O4) — readings S5-S8 in DESIGN.md.
+
+The paper gives Eq.13-15 (L239-249) and the statement that chemistry is explicit and sub-cycled
+(L87); what is pinned here is (i) the rate fits against textbook values, (ii) the algebra of the
+backward-Euler sub-step against a brute-force bisection of the same implicit system, (iii) exact
+photon/energy budgets and (iv) the closed-form equilibria of Eq.14.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+C = 2.99792458e10
+KB = 1.380649e-16
+EV = 1.602176634e-12
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _params(orc, **kw):
+    from paper_1004_2503_b200.workloads import default_params
+    p = default_params()
+    nH_mean = kw.pop("nH_mean", 1.0)
+    p.update(kw)
+    return orc.make_params(p, 1.0e21, nH_mean)
+
+
+# ------------------------------------------------------------------ rate fits (S7)
+def test_recombination_fits_match_textbook_table(orc):
+    rows = [l.split() for l in open(os.path.join(GOLD, "osterbrock_recombination.txt"))
+            if l.strip() and not l.startswith("#")]
+    for T, aA, aB in rows:
+        r = orc.rates(float(T))
+        assert r["alpha_A"] == pytest.approx(float(aA), rel=0.03)
+        assert r["alpha_B"] == pytest.approx(float(aB), rel=0.03)
+    # the Stroemgren test's alpha_B (north_star): 2.59e-13 at 1e4 K
+    assert orc.rates(1e4)["alpha_B"] == pytest.approx(2.59e-13, rel=2e-3)
+
+
+def test_collisional_and_cooling_fits_orders_of_magnitude(orc):
+    """Independent (different-author) closed forms: Voronov (1997) for the collisional ionisation
+    rate (within 25 %), Cen (1992) for the cooling rates (within a factor 2) over 1e4-1e6 K;
+    z_ci = 13.6 eV * beta exactly; the Boltzmann factors kill the rates in cold gas."""
+    for T in (1e4, 3e4, 1e5, 1e6):
+        r = orc.rates(T)
+        U = 13.6 * EV / (KB * T)
+        voronov = 2.91e-8 * U ** 0.39 * math.exp(-U) / (0.232 + U)
+        assert 0.75 < r["beta"] / voronov < 1.25
+        assert r["z_ci"] == pytest.approx(13.6 * EV * r["beta"], rel=1e-14)
+        cen_rec = 8.70e-27 * math.sqrt(T) * (T / 1e3) ** -0.2 / (1 + (T / 1e6) ** 0.7)
+        if T <= 3e4:                                  # Cen's fit is only good near 1e4 K
+            assert 0.5 < r["z_recA"] / cen_rec < 2.0
+        assert 0.2 < r["z_recA"] / (r["alpha_A"] * KB * T) < 1.5
+        assert r["z_recB"] < r["z_recA"]
+        assert r["alpha_B"] < r["alpha_A"]
+        # mean kinetic energy lost per case-B recombination is of order kT
+        assert 0.2 < r["z_recB"] / (r["alpha_B"] * KB * T) < 1.5
+        cen_ff = 1.42e-27 * math.sqrt(T) * 1.3
+        assert 0.8 < r["z_ff"] / cen_ff < 1.2
+    cold = orc.rates(100.0)
+    assert cold["beta"] == 0.0 and cold["z_exc"] == 0.0      # exp(-1578) underflows even in fp64
+
+
+@pytest.mark.parametrize("T", [50.0, 3e3, 1.2e4, 8e4, 2e6])
+def test_log_derivatives_match_finite_differences(orc, T):
+    h = 1e-5
+    rp, rm, r0 = orc.rates(T * math.exp(h)), orc.rates(T * math.exp(-h)), orc.rates(T)
+    for z, dl in (("z_recA", "dl_recA"), ("z_recB", "dl_recB"), ("z_ci", "dl_ci"),
+                  ("z_exc", "dl_exc"), ("z_ff", "dl_ff")):
+        if r0[z] == 0.0:
+            continue
+        fd = (math.log(rp[z]) - math.log(rm[z])) / (2 * h)
+        assert r0[dl] == pytest.approx(fd, rel=1e-6, abs=1e-7)
+
+
+def test_clumping_laws(orc):
+    p = _params(orc, clump_model=0)
+    assert orc.clumping(5.0, p) == 1.0
+    p = _params(orc, clump_model=1, clump_a=1.0, clump_b=2.0, nH_mean=2.0)   # C = max(1, 1 + 2 delta)
+    assert orc.clumping(6.0, p) == pytest.approx(1 + 2 * (6.0 / 2.0 - 1))
+    assert orc.clumping(0.5, p) == 1.0                                         # 1+2 delta < 1 clamps
+    p = _params(orc, clump_model=2, clump_a=30.0, clump_b=0.7)                 # K nH^0.7 (L259)
+    assert orc.clumping(0.1, p) == pytest.approx(30.0 * 0.1 ** 0.7)
+
+
+# ------------------------------------------------------------------ the backward-Euler sub-step
+def _draw(rng):
+    nH = 10 ** rng.uniform(-6, 0)
+    return dict(N=10 ** rng.uniform(-12, 1) * nH * rng.choice([0, 1, 1, 1]),
+                x=rng.choice([10 ** rng.uniform(-6, -0.01), 1 - 10 ** rng.uniform(-7, -1)]),
+                T=10 ** rng.uniform(1.5, 6), nH=nH, dts=10 ** rng.uniform(8, 13))
+
+
+def _implicit_residual(yp, d, p, r, CR, case_b, coll):
+    """x' - x - dts[ y'(c sigma N' + beta n_e) - alpha C_R n_e x' ], N' from backward Euler."""
+    x, y = d["x"], 1 - d["x"]
+    ne = x * d["nH"]
+    alpha = r["alpha_B"] if case_b else r["alpha_A"]
+    beta = r["beta"] if coll else 0.0
+    S = 0.0 if case_b else (r["alpha_A"] - r["alpha_B"]) * CR * ne * x * d["nH"]
+    A = p.c * p.sigma_n * d["nH"] * d["dts"]
+    Np = (d["N"] + d["dts"] * S) / (1 + A * yp)
+    xp = 1 - yp
+    return (xp - x) - d["dts"] * (yp * (p.c * p.sigma_n * Np + beta * ne) - alpha * CR * ne * xp), Np
+
+
+@pytest.mark.parametrize("case_b,coll,clump", [(1, 1, 0), (0, 1, 1), (1, 0, 0), (0, 0, 1)])
+def test_substep_solves_the_implicit_system_and_conserves_photons(orc, case_b, coll, clump):
+    """P5: the closed-form quadratic root equals the unique root in (0,1] of the backward-Euler
+    system found by bisection; and N' + nH x' = N + nH x + dts S_rec + nH (b y' - r x') exactly."""
+    rng = np.random.default_rng(10 + case_b * 2 + coll)
+    p = _params(orc, recomb_case=case_b, coll_ion=coll, clump_model=clump, cooling=0, nH_mean=1e-3)
+    for _ in range(400):
+        d = _draw(rng)
+        r = orc.rates(d["T"])
+        CR = orc.clumping(d["nH"], p)
+        F0 = np.array([0.3, -0.2, 0.1]) * C * d["N"]
+        Nn, Fn, xn, Tn, absorbed = orc.chem_substep(d["N"], F0, d["x"], d["T"], d["nH"], d["dts"], p)
+        assert 0.0 <= xn <= 1.0 and Nn >= 0.0 and Tn == d["T"]
+        # brute force: bisection on y' in [0, 1]
+        lo, hi = 0.0, 1.0
+        flo = _implicit_residual(lo, d, p, r, CR, case_b, coll)[0]
+        fhi = _implicit_residual(hi, d, p, r, CR, case_b, coll)[0]
+        assert flo >= 0 >= fhi
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            if _implicit_residual(mid, d, p, r, CR, case_b, coll)[0] > 0:
+                lo = mid
+            else:
+                hi = mid
+        yb = 0.5 * (lo + hi)
+        Nb = _implicit_residual(yb, d, p, r, CR, case_b, coll)[1]
+        assert (1 - xn) == pytest.approx(yb, rel=1e-7, abs=1e-13)
+        assert Nn == pytest.approx(Nb, rel=1e-6, abs=1e-300)
+        # photon budget identity
+        ne = d["x"] * d["nH"]
+        alpha = r["alpha_B"] if case_b else r["alpha_A"]
+        b = d["dts"] * (r["beta"] if coll else 0.0) * ne
+        rr = d["dts"] * alpha * CR * ne
+        S = 0.0 if case_b else (r["alpha_A"] - r["alpha_B"]) * CR * ne * d["x"] * d["nH"]
+        lhs = Nn + d["nH"] * xn
+        rhs = d["N"] + d["nH"] * d["x"] + d["dts"] * S + d["nH"] * (b * (1 - xn) - rr * xn)
+        assert lhs == pytest.approx(rhs, rel=1e-10)
+        assert absorbed == pytest.approx(d["N"] + d["dts"] * S - Nn, rel=1e-6, abs=1e-14 * d["nH"])
+        # flux attenuated by 1/(1 + A y'): same factor as N when S_rec = 0 (f unchanged)
+        if d["N"] > 0:
+            assert np.allclose(Fn / F0, Nn / (d["N"] + d["dts"] * S), rtol=1e-12)
+        A = p.c * p.sigma_n * d["nH"] * d["dts"]
+        assert np.allclose(Fn, F0 / (1 + A * (1 - xn)), rtol=1e-5)
+
+
+def test_absorbed_photons_equal_ionisations_without_recombination(orc):
+    """With alpha -> 0 (very hot gas, tiny n_e) and beta = 0 every absorbed photon ionises one atom."""
+    p = _params(orc, coll_ion=0, cooling=0)
+    N, x, nH, dts = 3e-6, 1e-9, 1e-4, 1e10
+    Nn, _, xn, _, ab = orc.chem_substep(N, [0, 0, 0], x, 1e9, nH, dts, p)
+    assert (xn - x) * nH == pytest.approx(N - Nn, rel=1e-6)
+    assert ab == pytest.approx(N - Nn, rel=1e-12)
+
+
+@pytest.mark.parametrize("clump", [0, 1])
+def test_photoionisation_equilibrium_closed_form(orc, clump):
+    """P6 / PAPER.md:L229-231, Eq.14: the steady state satisfies alpha C_R nH x^2 =
+    (1-x)(c sigma_n N + beta nH x) whatever dts; optically thin it is the closed-form root."""
+    p = _params(orc, cooling=0, coll_ion=1, clump_model=clump, nH_mean=1e-4)
+    nH, T, N0 = 3e-4, 2.0e4, 1e-9
+    r = orc.rates(T)
+    CR = orc.clumping(nH, p)
+    assert CR == pytest.approx(5.0 if clump else 1.0, rel=1e-14)
+    for dts in (1e9, 1e11, 3e12):
+        x = 0.3
+        for _ in range(20000):
+            Nn, _, x, _, _ = orc.chem_substep(N0, [0, 0, 0], x, T, nH, dts, p)
+        G = p.c * p.sigma_n * Nn
+        assert r["alpha_B"] * CR * nH * x * x == pytest.approx((1 - x) * (G + r["beta"] * nH * x), rel=1e-9)
+    # optically thin limit (tiny cross-section, photons >> atoms absorbed per step): N' ~ N0 and the
+    # fixed point is the closed-form root of  (alpha C_R + beta) nH x^2 + (G - beta nH) x - G = 0
+    p = _params(orc, cooling=0, coll_ion=1, clump_model=clump, nH_mean=1e-4, sigma_n=1e-24, sigma_e=1e-24)
+    nH, N0 = 1e-3, 5e-3 * (5.0 if clump else 1.0)
+    CR = orc.clumping(nH, p)
+    a = (r["alpha_B"] * CR + r["beta"]) * nH
+    G0 = p.c * p.sigma_n * N0
+    bq = G0 - r["beta"] * nH
+    x_eq = (-bq + math.sqrt(bq * bq + 4 * a * G0)) / (2 * a)
+    assert 0.2 < x_eq < 0.99
+    dts = 1.4e13 / CR
+    x = 0.5
+    for _ in range(30000):
+        Nn, _, x, _, _ = orc.chem_substep(N0, [0, 0, 0], x, T, nH, dts, p)
+    A_y = p.c * p.sigma_n * nH * dts * (1 - x)
+    assert A_y < 1e-3
+    assert x == pytest.approx(x_eq, rel=2 * A_y + 1e-9)
+
+
+def test_thermal_fixed_point_heating_equals_cooling(orc):
+    """P6 (thermal): iterate Phi at fixed N until (x,T) stop changing; then photo-heating equals the
+    cooling function evaluated from the rate fits."""
+    p = _params(orc, cooling=1, coll_ion=1, redshift=-1.0)
+    nH, N0, dt = 1e-1, 1e-6, 3e11
+    x, T = 0.5, 1.0e4
+    for _ in range(40000):
+        _, _, x, T, _ = orc.chem_cell(N0, [0, 0, 0], x, T, nH, dt, p)
+    x1, T1 = x, T
+    Nn, _, x, T, ab = orc.chem_substep(N0, [0, 0, 0], x1, T1, nH, dt, p)
+    assert x == pytest.approx(x1, rel=1e-9) and T == pytest.approx(T1, rel=1e-9)
+    r = orc.rates(T1)
+    lam = nH * nH * (x1 * x1 * (r["z_recB"] + r["z_ff"]) + x1 * (1 - x1) * (r["z_exc"] + r["z_ci"]))
+    heat = ab / dt * (p.e_photon_eV * p.sigma_e / p.sigma_n - 13.6) * EV
+    assert heat == pytest.approx(lam, rel=1e-6)
+    assert 5e3 < T1 < 5e4                      # photo-heated gas sits at ~1e4 K
+
+
+def test_energy_update_and_subcycling(orc):
+    """Pure photo-heating (no cooling-relevant species: x tiny, cold): dE = absorbed*(e sigma_e/sigma_n - e0);
+    isothermal mode is exactly one sub-step; sub-steps add up to dt and obey the 10 % rule."""
+    p = _params(orc, cooling=1, coll_ion=0)
+    nH, x, T, N, dts = 1e-3, 1e-4, 50.0, 1e-12, 1e9
+    Nn, _, xn, Tn, ab = orc.chem_substep(N, [0, 0, 0], x, T, nH, dts, p)
+    E0 = 1.5 * KB * nH * (1 + x) * T
+    E1 = 1.5 * KB * nH * (1 + xn) * Tn
+    r = orc.rates(T)
+    lam = nH * nH * (xn * xn * (r["z_recB"] + r["z_ff"]))          # exc/ci are exactly 0 at 50 K
+    lam_T = nH * nH * xn * xn * (r["z_recB"] * r["dl_recB"] + r["z_ff"] * r["dl_ff"])
+    want = E0 + (ab * (p.e_photon_eV - 13.6) * EV - dts * lam) / (1 + dts * max(0, lam_T) / E0)
+    assert E1 == pytest.approx(want, rel=1e-12)
+    assert ab * (p.e_photon_eV - 13.6) * EV > 100 * dts * lam          # heating dominates here
+    # isothermal: chem_cell == one substep
+    q = _params(orc, cooling=0)
+    a = orc.chem_cell(1e-6, [1e3, 0, 0], 0.2, 1e4, 1e-3, 1e11, q)
+    b = orc.chem_substep(1e-6, [1e3, 0, 0], 0.2, 1e4, 1e-3, 1e11, q)
+    assert a[4] == 1 and a[0] == b[0] and a[2] == b[2] and a[3] == 1e4
+    # strong source: many sub-cycles, each changing E by about <= 10 % (estimated rate is lagged)
+    N, F, x, T = 1e-2, np.zeros(3), 1.2e-3, 100.0
+    Nn, _, xn, Tn, ns = orc.chem_cell(N, F, x, T, 1e-3, 5.6e9, p)
+    assert ns > 5
+    # energy conservation over the sub-cycled step when cooling is negligible vs heating
+    assert Tn > 1e3 and 0 < xn <= 1
+    # max_sub cap is honoured
+    q = _params(orc, cooling=1, max_sub=3)
+    assert orc.chem_cell(N, F, x, T, 1e-3, 5.6e9, q)[4] == 3
+
+
+def test_subcycled_result_converges_with_tolerance(orc):
+    """The sub-cycled operator converges as eps_sub -> 0 (first order): halving eps halves the
+    distance to the eps -> 0 limit."""
+    res = []
+    for eps in (0.2, 0.1, 0.05, 0.003125):
+        p = _params(orc, cooling=1, eps_sub=eps)
+        res.append(orc.chem_cell(3e-4, [0, 0, 0], 0.01, 300.0, 1e-3, 2e10, p))
+    Tref = res[-1][3]
+    e = [abs(r[3] - Tref) for r in res[:3]]
+    assert e[0] > e[1] > e[2]
+    assert e[1] / e[2] == pytest.approx(2.0, rel=0.35)
