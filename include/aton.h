@@ -1,0 +1,131 @@
+/*
+ * aton.h -- C ABI of the B200-native ATON hot path.
+ *
+ * The operation is the explicit moment radiative-transfer step of Aubert & Teyssier,
+ * "Reionization simulations powered by GPUs I" on a uniform periodic 3-D grid:
+ *   transport of the photon density N and flux F with the M1 closure and a Lax-Friedrichs
+ *   intercell flux (Eq.3-7; appendix Eq.A1-A5), then per cell the
+ *   source term and the sub-cycled hydrogen photo-chemistry / cooling operator Phi of Eq.A4
+ *   (Eq.13-15), in the order "transport, then the chemistry
+ *   and the cooling".
+ * The host only drives: fields go up once, every step runs on the GPU, fields
+ * and the global means of PAPER.md:L149/L303 come back on request.
+ *
+ * All entry points are plain C.  No call aborts or throws; each returns ATON_OK (0) or a negative
+ * code and leaves a message in aton_last_error().  Calls on one context are not thread-safe;
+ * different contexts are independent.  Everything runs on the CUDA stream given to aton_init
+ * (a cudaStream_t cast to void*, NULL = the legacy default stream) on the device that is current
+ * at aton_init.  There is no CPU fallback: without a CUDA device aton_init returns ATON_ECUDA.
+ *
+ * Layout of every field: C order [nz][ny][nx], x fastest; cell (i,j,k) at i + nx*(j + ny*k);
+ * float32; cubic cells dx = lx_cm/nx; periodic in x, y and z (wrapped in-kernel, no ghost layer).
+ * Units are CGS: n_H, N [cm^-3]; F [photons cm^-2 s^-1]; T [K]; x = n_HII/n_H; rate [photons/s];
+ * dt [s].  Pointers are host or device pointers as said by the `on_device` argument; the caller
+ * owns every array it passes, the library copies and never keeps a caller pointer.
+ */
+#ifndef ATON_H
+#define ATON_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ATON_OK 0
+#define ATON_EINVAL (-1) /* bad argument: NULL, bad grid, unstable dt, position outside [0,1], ... */
+#define ATON_ENOMEM (-2) /* device or host allocation failed */
+#define ATON_ECUDA (-3)  /* CUDA error (sticky; text in aton_last_error) */
+#define ATON_ESTATE (-4) /* call out of order, e.g. aton_step before aton_set_fields */
+
+typedef struct aton_ctx aton_t; /* opaque; owned by the library, released by aton_free */
+
+/* nx % 4 == 0 (128-bit accesses along x), ny, nz >= 1; nx*ny*nz < 2^31. */
+typedef struct { int nx, ny, nz; } aton_grid_t;
+
+/* Physical side along x in cm.  Cells are cubic: dx = lx_cm / nx. */
+typedef struct { double lx_cm; } aton_box_t;
+
+/* Units and physics switches.  Zero-initialise, then set; 0 means "default" where noted. */
+typedef struct {
+    double c_cm_s;       /* speed of light of the transport; 0 => 2.99792458e10 ("c full speed") */
+    double sigma_n;      /* number-averaged photoionisation cross-section, cm^2 (2.93e-18) */
+    double sigma_e;      /* energy-averaged cross-section, cm^2 (2.49e-18) */
+    double e_photon_eV;  /* mean ionising photon energy, eV (20.27) */
+    int recomb_case;     /* 1: case B (on-the-spot); 0: case A + recombination radiation */
+    int cooling;         /* 0: T frozen (isothermal); 1: photo-heating + cooling, sub-cycled */
+    int coll_ion;        /* collisional ionisation and its cooling on/off */
+    int clump_model;     /* recombination clumping C_R of Eq.15:
+                            0 none; 1: C = max(1, a + b*delta), delta = n_H/<n_H> - 1;
+                            2: C = max(1, a * n_H^b) (PAPER.md:L259 power law) */
+    double clump_a, clump_b;
+    double redshift;     /* >= 0: Compton cooling off the CMB at this z; < 0: off */
+    double eps_sub;      /* sub-cycle tolerance on the thermal energy change; 0 => 0.1 */
+    int max_sub;         /* sub-cycle cap per cell and step; 0 => 16384 */
+} aton_params_t;
+
+/* Global diagnostics (PAPER.md:L149 volume-weighted x, L303-305 mass-weighted, Eq.15 Gamma = c sigma_n N). */
+typedef struct {
+    double x_vol, x_mass;         /* <x>_V = mean x ; <x>_M = sum(n_H x)/sum(n_H) */
+    double gamma_vol, gamma_mass; /* photo-ionisation rate c*sigma_n*N [1/s], volume / mass weighted */
+    double photons_total;         /* sum N dx^3 */
+    double T_vol;                 /* mean T */
+    double f_max;                 /* max reduced flux |F|/(cN) over cells with N > 0 */
+    double N_min;                 /* min N */
+    double frac_x_half;           /* fraction of cells with x >= 0.5 */
+    long long n_nonfinite;        /* cells holding a NaN/Inf in any of N, F, x, T */
+    long long subcycles_total;    /* chemistry sub-cycles summed over cells and steps since aton_set_fields */
+    long long subcycles_max;      /* largest per-cell, per-step sub-cycle count seen */
+    long long steps_done;         /* steps since aton_set_fields */
+    double time_s;                /* sum of dt since aton_set_fields */
+} aton_diag_t;
+
+/* Create a context: allocates 11 float32 device arrays of nx*ny*nz (7 fields + 4 ping-pong).
+ * `stream` is borrowed for the life of the context.  On failure *out is NULL. */
+int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box,
+              const aton_params_t *params, void *cuda_stream);
+
+/* Upload the state {n_H, x, T, N, F}.  N, Fx, Fy, Fz may each be NULL = zero
+ * (dark start).  n_H must be > 0 everywhere (checked: ATON_EINVAL).  Resets the step counter, the
+ * sub-cycle statistics and <n_H> of the clumping law.  Synchronises the stream. */
+int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T, const float *N,
+                    const float *Fx, const float *Fy, const float *Fz, int on_device);
+
+/* Replace the source list (n = 0 clears it).  pos: n x 3 floats (x,y,z) in box units [0,1];
+ * rate: n doubles, photons/s, >= 0.  Nearest-grid-point: cell = floor(pos*n) mod n per axis, one
+ * emitter per cell, rates of sources sharing a cell are summed.  Synchronises. */
+int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *rate, int on_device);
+
+/* courant * dx / (3c): the unsplit 3-D Lax-Friedrichs step is stable for c*dt/dx <= 1/3
+ * (Eq.7 L80-83 gives dt < dx/c; reading S3).  Negative on a NULL context. */
+double aton_courant_dt(const aton_t *ctx, double courant);
+
+/* Advance n_steps steps of size dt [s] (dt <= 0 => aton_courant_dt(ctx, 0.8)).  Each step:
+ * transport -> source injection -> chemistry/cooling.  Asynchronous on the stream; the state at
+ * t + n_steps*dt is current afterwards whatever the parity of n_steps.  ATON_EINVAL if
+ * c*dt/dx > 1/3 or n_steps < 0; ATON_ESTATE before aton_set_fields. */
+int aton_step(aton_t *ctx, double dt, int n_steps);
+
+/* Download the state.  Any pointer may be NULL = skip.  Synchronises the stream. */
+int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float *Fx, float *Fy,
+                    float *Fz, int on_device);
+
+/* Global diagnostics of the current state (deterministic two-pass reduction).  Synchronises. */
+int aton_reduce(aton_t *ctx, aton_diag_t *out);
+
+/* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
+ * memory); 1 = tiled streaming kernel (default).  tile_y / tile_z choose the tile shape of
+ * variant 1 (0 = default); results do not depend on the tile shape. */
+int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
+
+/* Number of kernels launched by the library on this context since aton_init. */
+long long aton_launch_count(const aton_t *ctx);
+
+void aton_free(aton_t *ctx);
+
+/* Message of the last failing call on ctx (ctx-owned), or of the last failing aton_init if ctx is
+ * NULL (static storage).  Never NULL. */
+const char *aton_last_error(const aton_t *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ATON_H */

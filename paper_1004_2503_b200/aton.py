@@ -1,0 +1,198 @@
+"""Thin ctypes binding of the C ABI in include/aton.h: argument marshalling only.
+
+Every step of the path runs in libaton.so's CUDA kernels.  torch supplies device memory for the
+caller-side tensors and the CUDA stream.  There is no CPU fallback: a missing library or a machine
+without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaton.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+
+EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt", "aton_step",
+           "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_free",
+           "aton_last_error")
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int)]
+
+
+class Box(C.Structure):
+    _fields_ = [("lx_cm", C.c_double)]
+
+
+class Params(C.Structure):
+    _fields_ = [("c_cm_s", C.c_double), ("sigma_n", C.c_double), ("sigma_e", C.c_double),
+                ("e_photon_eV", C.c_double), ("recomb_case", C.c_int), ("cooling", C.c_int),
+                ("coll_ion", C.c_int), ("clump_model", C.c_int), ("clump_a", C.c_double),
+                ("clump_b", C.c_double), ("redshift", C.c_double), ("eps_sub", C.c_double),
+                ("max_sub", C.c_int)]
+
+
+class Diag(C.Structure):
+    _fields_ = [("x_vol", C.c_double), ("x_mass", C.c_double), ("gamma_vol", C.c_double),
+                ("gamma_mass", C.c_double), ("photons_total", C.c_double), ("T_vol", C.c_double),
+                ("f_max", C.c_double), ("N_min", C.c_double), ("frac_x_half", C.c_double),
+                ("n_nonfinite", C.c_longlong), ("subcycles_total", C.c_longlong),
+                ("subcycles_max", C.c_longlong), ("steps_done", C.c_longlong), ("time_s", C.c_double)]
+
+
+class AtonError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"aton error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libaton.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not found: build it with `python -m paper_1004_2503_b200.build` "
+                                "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp, fp, dp = C.c_void_p, C.c_void_p, C.c_void_p
+    L.aton_init.restype = C.c_int
+    L.aton_init.argtypes = [C.POINTER(vp), C.POINTER(Grid), C.POINTER(Box), C.POINTER(Params), vp]
+    L.aton_set_fields.restype = C.c_int
+    L.aton_set_fields.argtypes = [vp] + [fp] * 7 + [C.c_int]
+    L.aton_set_sources.restype = C.c_int
+    L.aton_set_sources.argtypes = [vp, C.c_longlong, fp, dp, C.c_int]
+    L.aton_courant_dt.restype = C.c_double
+    L.aton_courant_dt.argtypes = [vp, C.c_double]
+    L.aton_step.restype = C.c_int
+    L.aton_step.argtypes = [vp, C.c_double, C.c_int]
+    L.aton_get_fields.restype = C.c_int
+    L.aton_get_fields.argtypes = [vp] + [fp] * 7 + [C.c_int]
+    L.aton_reduce.restype = C.c_int
+    L.aton_reduce.argtypes = [vp, C.POINTER(Diag)]
+    L.aton_set_kernel.restype = C.c_int
+    L.aton_set_kernel.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+    L.aton_launch_count.restype = C.c_longlong
+    L.aton_launch_count.argtypes = [vp]
+    L.aton_free.restype = None
+    L.aton_free.argtypes = [vp]
+    L.aton_last_error.restype = C.c_char_p
+    L.aton_last_error.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def make_params(d: Dict[str, float]) -> Params:
+    p = Params()
+    for k, _ in Params._fields_:
+        if k in d:
+            setattr(p, k, type(getattr(p, k))(d[k]))
+    return p
+
+
+def _ptr(t: Optional[torch.Tensor], n: int, dtype, want_cuda: bool):
+    if t is None:
+        return None
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() != n:
+        raise ValueError(f"expected a contiguous {dtype} tensor of {n} elements")
+    if t.is_cuda != want_cuda:
+        raise ValueError("all tensors of one call must live on the same side (host or device)")
+    return C.c_void_p(t.data_ptr())
+
+
+class Aton:
+    """One simulation context (aton_t).  Methods mirror the C entry points one to one."""
+
+    def __init__(self, nx: int, ny: int, nz: int, lx_cm: float, params: Dict[str, float],
+                 stream: Optional[torch.cuda.Stream] = None):
+        self._L = load_library()
+        self._h = C.c_void_p()
+        self.shape = (nz, ny, nx)
+        self.ncell = nx * ny * nz
+        self._stream = stream
+        sp = C.c_void_p(stream.cuda_stream if stream is not None
+                        else (torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0))
+        g, b, p = Grid(nx, ny, nz), Box(lx_cm), make_params(params)
+        rc = self._L.aton_init(C.byref(self._h), C.byref(g), C.byref(b), C.byref(p), sp)
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise AtonError(rc, self._L.aton_last_error(None).decode())
+
+    # -- plumbing
+    def _check(self, rc: int):
+        if rc != OK:
+            raise AtonError(rc, self._L.aton_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._L.aton_free(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C entry points
+    def set_fields(self, nH, x, T, N=None, Fx=None, Fy=None, Fz=None):
+        dev = nH.is_cuda
+        ptrs = [_ptr(t, self.ncell, torch.float32, dev) for t in (nH, x, T, N, Fx, Fy, Fz)]
+        self._check(self._L.aton_set_fields(self._h, *ptrs, int(dev)))
+
+    def set_sources(self, pos: Optional[torch.Tensor], rate: Optional[torch.Tensor]):
+        n = 0 if rate is None else rate.numel()
+        if n == 0:
+            self._check(self._L.aton_set_sources(self._h, 0, None, None, 0))
+            return
+        dev = pos.is_cuda
+        self._check(self._L.aton_set_sources(self._h, n, _ptr(pos, 3 * n, torch.float32, dev),
+                                             _ptr(rate, n, torch.float64, dev), int(dev)))
+
+    def courant_dt(self, courant: float = 0.8) -> float:
+        return float(self._L.aton_courant_dt(self._h, courant))
+
+    def step(self, dt: float, n_steps: int = 1):
+        self._check(self._L.aton_step(self._h, float(dt), int(n_steps)))
+
+    def get_fields(self, device=None, names=("nH", "x", "T", "N", "Fx", "Fy", "Fz"), out=None) -> Dict[str, torch.Tensor]:
+        """Download the named fields into new tensors (on `device`, default cuda) or into `out`."""
+        order = ("nH", "x", "T", "N", "Fx", "Fy", "Fz")
+        if out is None:
+            device = torch.device(device or "cuda")
+            out = {k: torch.empty(self.shape, dtype=torch.float32, device=device,
+                                  pin_memory=(device.type == "cpu")) for k in names}
+        dev = next(iter(out.values())).is_cuda
+        ptrs = [_ptr(out.get(k), self.ncell, torch.float32, dev) if k in out else None for k in order]
+        self._check(self._L.aton_get_fields(self._h, *ptrs, int(dev)))
+        return out
+
+    def reduce(self) -> Dict[str, float]:
+        d = Diag()
+        self._check(self._L.aton_reduce(self._h, C.byref(d)))
+        return {k: getattr(d, k) for k, _ in Diag._fields_}
+
+    def set_kernel(self, variant: int, tile_y: int = 0, tile_z: int = 0):
+        self._check(self._L.aton_set_kernel(self._h, variant, tile_y, tile_z))
+
+    def launch_count(self) -> int:
+        return int(self._L.aton_launch_count(self._h))
+
+
+def from_workload(w, stream=None, device="cuda") -> Aton:
+    """Context initialised from a workloads.Workload (fields uploaded, sources set)."""
+    a = Aton(w.n, w.n, w.n, w.box_cm, w.params, stream)
+    f = [t.to(device).contiguous() for t in w.fields()]
+    a.set_fields(*f)
+    a.set_sources(w.src_pos.contiguous(), w.src_rate.contiguous())
+    return a

@@ -1,0 +1,428 @@
+// C ABI of the ATON hot path (include/aton.h): context, uploads/downloads, source lists, the step
+// loop and the diagnostics.  The host only drives; every step of the path runs in
+// the kernels of aton_step_tiled.cuh / aton_step_ref.cuh / aton_reduce.cuh.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/aton.h"
+#include "aton_physics.cuh"
+#include "aton_reduce.cuh"
+#include "aton_step_ref.cuh"
+#include "aton_step_tiled.cuh"
+
+using namespace aton;
+
+namespace {
+
+constexpr double K_BOLTZ = 1.380649e-16, EV_ERG = 1.602176634e-12, E0_EV = 13.6;
+constexpr int REDUCE_BLOCKS = 148 * 8;
+
+char g_init_error[512] = "";
+
+}  // namespace
+
+struct aton_ctx {
+    Grid g{};
+    size_t ncell = 0;
+    double dx = 0, c = 0;
+    aton_params_t p{};
+    cudaStream_t stream = nullptr;
+    float *rad[2][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
+    float *x = nullptr, *T = nullptr, *nH = nullptr;
+    int cur = 0;
+    unsigned *src_mask = nullptr;
+    int *src_cell = nullptr;
+    float *src_rho = nullptr;
+    int n_src = 0;
+    unsigned long long *stats = nullptr;   // device [2]
+    double *partials = nullptr;            // device [REDUCE_BLOCKS+1][R_COUNT]
+    double nH_mean = 1.0;
+    bool have_fields = false;
+    long long steps_done = 0, launches = 0;
+    double time_s = 0;
+    int variant = 0, tile_y = 0, tile_z = 0;
+    char err[512] = "";
+};
+
+namespace {
+
+int fail(aton_ctx *ctx, int code, const char *fmt, ...) {
+    char *dst = ctx ? ctx->err : g_init_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(ctx, call)                                                                         \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,      \
+                        "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+int flags_of(const aton_params_t &p) {
+    return (p.recomb_case == 0 ? F_CASE_A : 0) | (p.cooling ? F_COOL : 0) | (p.coll_ion ? F_COLL : 0);
+}
+
+StepConst make_step_const(const aton_ctx *ctx, double dt) {
+    const aton_params_t &p = ctx->p;
+    const double kb15 = 1.5 * K_BOLTZ;
+    StepConst s{};
+    const double h = ctx->c * dt / (2.0 * ctx->dx);
+    s.h = (float)h;
+    s.keep = (float)(1.0 - 6.0 * h);
+    s.dt = (float)dt;
+    s.cs = (float)(ctx->c * p.sigma_n);
+    s.heat_K = (float)((p.e_photon_eV * p.sigma_e / p.sigma_n - E0_EV) * EV_ERG / kb15);
+    s.heat_rate_K = (float)(ctx->c * (p.e_photon_eV * p.sigma_e - E0_EV * p.sigma_n) * EV_ERG / kb15);
+    s.l2_zrec0 = (float)std::log2((p.recomb_case == 0 ? 1.778e-29 : 3.435e-30) / kb15);
+    s.zff0 = (float)(1.42e-27 / kb15);
+    s.zexc0 = (float)(7.5e-19 / kb15);
+    s.l2_zci0 = (float)std::log2(E0_EV * EV_ERG * 21.11 / kb15);
+    const double zp1 = 1.0 + p.redshift;
+    s.compton0 = p.redshift >= 0.0 ? (float)(5.65e-36 * zp1 * zp1 * zp1 * zp1 / kb15) : 0.0f;
+    s.t_cmb = (float)(2.726 * zp1);
+    s.eps_sub = (float)p.eps_sub;
+    s.max_sub = p.max_sub;
+    s.clump_model = p.clump_model;
+    if (p.clump_model == 1) {
+        s.clump_k0 = (float)(p.clump_a - p.clump_b);
+        s.clump_k1 = (float)(p.clump_b / ctx->nH_mean);
+    } else {
+        s.clump_k0 = (float)p.clump_a;
+        s.clump_k1 = (float)p.clump_b;
+    }
+    s.inj_scale = 0.0f;
+    return s;
+}
+
+FieldsIO make_io(const aton_ctx *ctx) {
+    FieldsIO f{};
+    const int a = ctx->cur, b = 1 - ctx->cur;
+    f.N = ctx->rad[a][0]; f.Gx = ctx->rad[a][1]; f.Gy = ctx->rad[a][2]; f.Gz = ctx->rad[a][3];
+    f.N1 = ctx->rad[b][0]; f.Gx1 = ctx->rad[b][1]; f.Gy1 = ctx->rad[b][2]; f.Gz1 = ctx->rad[b][3];
+    f.x = ctx->x; f.T = ctx->T; f.nH = ctx->nH;
+    f.src_mask = ctx->src_mask; f.src_cell = ctx->src_cell; f.src_rho = ctx->src_rho;
+    f.n_src = ctx->n_src;
+    f.stats = ctx->stats;
+    return f;
+}
+
+template <int FLAGS>
+cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
+    if (ctx->variant == 0) {
+        const int threads = 256;
+        const unsigned blocks = (unsigned)((ctx->ncell + threads - 1) / threads);
+        step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc);
+        return cudaGetLastError();
+    }
+    return launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+}
+
+cudaError_t launch_step(aton_ctx *ctx, const StepConst &sc) {
+    const FieldsIO f = make_io(ctx);
+    ctx->launches++;
+    switch (flags_of(ctx->p)) {
+        case 0: return launch_one<0>(ctx, f, sc);
+        case 1: return launch_one<1>(ctx, f, sc);
+        case 2: return launch_one<2>(ctx, f, sc);
+        case 3: return launch_one<3>(ctx, f, sc);
+        case 4: return launch_one<4>(ctx, f, sc);
+        case 5: return launch_one<5>(ctx, f, sc);
+        case 6: return launch_one<6>(ctx, f, sc);
+        default: return launch_one<7>(ctx, f, sc);
+    }
+}
+
+int scale_into(aton_ctx *ctx, const float *in, float *out, float s) {
+    const int nquad = (int)(ctx->ncell / 4);
+    const int blocks = std::min((nquad + 255) / 256, 148 * 16);
+    scale_kernel<<<blocks, 256, 0, ctx->stream>>>((const float4 *)in, (float4 *)out, s, nquad);
+    ctx->launches++;
+    CU(ctx, cudaGetLastError());
+    return ATON_OK;
+}
+
+// run the two-pass reduction; host_out[R_COUNT]
+int run_reduce(aton_ctx *ctx, bool full, double *host_out) {
+    const int nquad = (int)(ctx->ncell / 4);
+    const int blocks = std::min((nquad + 255) / 256, REDUCE_BLOCKS);
+    float **r = ctx->rad[ctx->cur];
+    reduce_pass1<<<blocks, 256, 0, ctx->stream>>>(
+        full ? (const float4 *)r[0] : nullptr, (const float4 *)r[1], (const float4 *)r[2], (const float4 *)r[3],
+        (const float4 *)ctx->x, (const float4 *)ctx->T, (const float4 *)ctx->nH, nquad, ctx->partials);
+    CU(ctx, cudaGetLastError());
+    double *out = ctx->partials + (size_t)REDUCE_BLOCKS * R_COUNT;
+    reduce_pass2<<<1, 32, 0, ctx->stream>>>(ctx->partials, blocks, out);
+    CU(ctx, cudaGetLastError());
+    ctx->launches += 2;
+    CU(ctx, cudaMemcpyAsync(host_out, out, sizeof(double) * R_COUNT, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    return ATON_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, const aton_params_t *params,
+              void *cuda_stream) {
+    if (out) *out = nullptr;
+    if (!out || !grid || !box || !params) return fail(nullptr, ATON_EINVAL, "aton_init: NULL argument");
+    if (grid->nx < 4 || grid->nx % 4 != 0 || grid->ny < 1 || grid->nz < 1)
+        return fail(nullptr, ATON_EINVAL, "aton_init: need nx %% 4 == 0, nx >= 4, ny, nz >= 1 (got %d %d %d)",
+                    grid->nx, grid->ny, grid->nz);
+    const double ncell_d = (double)grid->nx * grid->ny * grid->nz;
+    if (ncell_d >= 2147483648.0) return fail(nullptr, ATON_EINVAL, "aton_init: nx*ny*nz must be < 2^31");
+    if (!(box->lx_cm > 0.0)) return fail(nullptr, ATON_EINVAL, "aton_init: lx_cm must be > 0");
+    if (!(params->sigma_n > 0.0) || !(params->sigma_e > 0.0) || !(params->e_photon_eV > 0.0))
+        return fail(nullptr, ATON_EINVAL, "aton_init: sigma_n, sigma_e, e_photon_eV must be > 0");
+    if (params->clump_model < 0 || params->clump_model > 2 || params->c_cm_s < 0.0 || params->eps_sub < 0.0 ||
+        params->max_sub < 0)
+        return fail(nullptr, ATON_EINVAL, "aton_init: bad clump_model / c / eps_sub / max_sub");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, ATON_ECUDA, "aton_init: no CUDA device (there is no CPU fallback)");
+    }
+    aton_ctx *ctx = new (std::nothrow) aton_ctx();
+    if (!ctx) return fail(nullptr, ATON_ENOMEM, "aton_init: host allocation failed");
+    ctx->g = Grid{grid->nx, grid->ny, grid->nz};
+    ctx->ncell = (size_t)ncell_d;
+    ctx->p = *params;
+    ctx->c = params->c_cm_s > 0.0 ? params->c_cm_s : 2.99792458e10;
+    if (ctx->p.eps_sub == 0.0) ctx->p.eps_sub = 0.1;
+    if (ctx->p.max_sub == 0) ctx->p.max_sub = 1 << 14;
+    ctx->dx = box->lx_cm / grid->nx;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    const size_t bytes = ctx->ncell * sizeof(float);
+    cudaError_t e = cudaSuccess;
+    float **slots[11] = {&ctx->rad[0][0], &ctx->rad[0][1], &ctx->rad[0][2], &ctx->rad[0][3], &ctx->rad[1][0],
+                         &ctx->rad[1][1], &ctx->rad[1][2], &ctx->rad[1][3], &ctx->x, &ctx->T, &ctx->nH};
+    for (int i = 0; i < 11 && e == cudaSuccess; i++) e = cudaMalloc((void **)slots[i], bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->partials, sizeof(double) * (REDUCE_BLOCKS + 1) * R_COUNT);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_mask, sizeof(unsigned) * (ctx->ncell / 1024 + 1));
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 2 * sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->ncell / 1024 + 1), ctx->stream);
+    if (e != cudaSuccess) {
+        int code = fail(nullptr, e == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,
+                        "aton_init: device allocation failed: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        aton_free(ctx);
+        return code;
+    }
+    *out = ctx;
+    return ATON_OK;
+}
+
+void aton_free(aton_t *ctx) {
+    if (!ctx) return;
+    for (int b = 0; b < 2; b++)
+        for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
+    cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
+    cudaFree(ctx->src_mask); cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
+    cudaFree(ctx->stats); cudaFree(ctx->partials);
+    delete ctx;
+}
+
+const char *aton_last_error(const aton_t *ctx) { return ctx ? ctx->err : g_init_error; }
+
+long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0; }
+
+int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
+    if (!ctx) return ATON_EINVAL;
+    if (variant < 0 || variant > 1) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0 or 1");
+    if (variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z))
+        return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
+    ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
+    return ATON_OK;
+}
+
+int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T, const float *N, const float *Fx,
+                    const float *Fy, const float *Fz, int on_device) {
+    if (!ctx) return ATON_EINVAL;
+    if (!nH || !x || !T) return fail(ctx, ATON_EINVAL, "aton_set_fields: nH, x and T are required");
+    const size_t bytes = ctx->ncell * sizeof(float);
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    ctx->have_fields = false;
+    ctx->cur = 0;
+    CU(ctx, cudaMemcpyAsync(ctx->nH, nH, bytes, kind, ctx->stream));
+    CU(ctx, cudaMemcpyAsync(ctx->x, x, bytes, kind, ctx->stream));
+    CU(ctx, cudaMemcpyAsync(ctx->T, T, bytes, kind, ctx->stream));
+    const float *rad_in[4] = {N, Fx, Fy, Fz};
+    const float inv_c = (float)(1.0 / ctx->c);
+    for (int v = 0; v < 4; v++) {
+        float *dst = ctx->rad[0][v];
+        if (!rad_in[v]) {
+            CU(ctx, cudaMemsetAsync(dst, 0, bytes, ctx->stream));
+        } else {
+            CU(ctx, cudaMemcpyAsync(dst, rad_in[v], bytes, kind, ctx->stream));
+            if (v > 0) {   // the device carries G = F/c
+                int rc = scale_into(ctx, dst, dst, inv_c);
+                if (rc) return rc;
+            }
+        }
+    }
+    CU(ctx, cudaMemsetAsync(ctx->stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    double red[R_COUNT];
+    int rc = run_reduce(ctx, false, red);
+    if (rc) return rc;
+    if (!(red[R_NHMIN] > 0.0) || !std::isfinite(red[R_M]))
+        return fail(ctx, ATON_EINVAL, "aton_set_fields: n_H must be finite and > 0 everywhere (min %g)", red[R_NHMIN]);
+    ctx->nH_mean = red[R_M] / (double)ctx->ncell;
+    ctx->steps_done = 0;
+    ctx->time_s = 0.0;
+    ctx->have_fields = true;
+    return ATON_OK;
+}
+
+int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *rate, int on_device) {
+    if (!ctx) return ATON_EINVAL;
+    if (n < 0 || (n > 0 && (!pos || !rate))) return fail(ctx, ATON_EINVAL, "aton_set_sources: bad arguments");
+    std::vector<float> hpos;
+    std::vector<double> hrate;
+    if (n > 0 && on_device) {
+        hpos.resize(3 * n); hrate.resize(n);
+        CU(ctx, cudaMemcpyAsync(hpos.data(), pos, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(ctx, cudaMemcpyAsync(hrate.data(), rate, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(ctx, cudaStreamSynchronize(ctx->stream));
+        pos = hpos.data(); rate = hrate.data();
+    }
+    // NGP binning: cell = floor(pos*n) mod n; merge sources sharing a cell (fp64)
+    std::vector<std::pair<int, double>> cells((size_t)n);
+    const int dims[3] = {ctx->g.nx, ctx->g.ny, ctx->g.nz};
+    for (long long s = 0; s < n; s++) {
+        int ijk[3];
+        for (int a = 0; a < 3; a++) {
+            const double q = (double)pos[3 * s + a];
+            if (!(q >= 0.0 && q <= 1.0)) return fail(ctx, ATON_EINVAL, "aton_set_sources: position %lld outside [0,1]", s);
+            long long v = (long long)std::floor(q * dims[a]);
+            ijk[a] = (int)(v % dims[a]);
+        }
+        if (!(rate[s] >= 0.0) || !std::isfinite(rate[s]))
+            return fail(ctx, ATON_EINVAL, "aton_set_sources: rate %lld must be finite and >= 0", s);
+        cells[s] = {ijk[0] + ctx->g.nx * (ijk[1] + ctx->g.ny * ijk[2]), rate[s]};
+    }
+    std::stable_sort(cells.begin(), cells.end(), [](const auto &a, const auto &b) { return a.first < b.first; });
+    std::vector<int> ucell;
+    std::vector<double> urate;
+    for (const auto &cr : cells) {
+        if (!ucell.empty() && ucell.back() == cr.first) urate.back() += cr.second;
+        else { ucell.push_back(cr.first); urate.push_back(cr.second); }
+    }
+    const size_t nu = ucell.size();
+    const size_t nwords = ctx->ncell / 1024 + 1;
+    std::vector<unsigned> mask(nwords, 0u);
+    std::vector<float> rho(nu);
+    const double inv_vol = 1.0 / (ctx->dx * ctx->dx * ctx->dx);
+    for (size_t s = 0; s < nu; s++) {
+        const unsigned seg = (unsigned)ucell[s] >> 5;
+        mask[seg >> 5] |= 1u << (seg & 31);
+        rho[s] = (float)(urate[s] * inv_vol);
+    }
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
+    ctx->src_cell = nullptr; ctx->src_rho = nullptr; ctx->n_src = 0;
+    CU(ctx, cudaMemcpyAsync(ctx->src_mask, mask.data(), sizeof(unsigned) * nwords, cudaMemcpyHostToDevice, ctx->stream));
+    if (nu > 0) {
+        CU(ctx, cudaMalloc((void **)&ctx->src_cell, sizeof(int) * nu));
+        CU(ctx, cudaMalloc((void **)&ctx->src_rho, sizeof(float) * nu));
+        CU(ctx, cudaMemcpyAsync(ctx->src_cell, ucell.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, ctx->stream));
+        CU(ctx, cudaMemcpyAsync(ctx->src_rho, rho.data(), sizeof(float) * nu, cudaMemcpyHostToDevice, ctx->stream));
+    }
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->n_src = (int)nu;
+    return ATON_OK;
+}
+
+double aton_courant_dt(const aton_t *ctx, double courant) {
+    if (!ctx) return -1.0;
+    return courant * ctx->dx / (3.0 * ctx->c);
+}
+
+int aton_step(aton_t *ctx, double dt, int n_steps) {
+    if (!ctx) return ATON_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_step: call aton_set_fields first");
+    if (n_steps < 0) return fail(ctx, ATON_EINVAL, "aton_step: n_steps < 0");
+    if (!(dt > 0.0)) dt = aton_courant_dt(ctx, 0.8);
+    const double mu = ctx->c * dt / ctx->dx;
+    if (!(mu <= (1.0 / 3.0) * (1.0 + 1e-12)) || !std::isfinite(mu))
+        return fail(ctx, ATON_EINVAL, "aton_step: c*dt/dx = %g > 1/3 is unstable for the unsplit 3-D LF scheme", mu);
+    const StepConst sc = make_step_const(ctx, dt);
+    for (int s = 0; s < n_steps; s++) {
+        CU(ctx, launch_step(ctx, sc));
+        ctx->cur = 1 - ctx->cur;
+        ctx->steps_done++;
+        ctx->time_s += dt;
+    }
+    return ATON_OK;
+}
+
+int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float *Fx, float *Fy, float *Fz,
+                    int on_device) {
+    if (!ctx) return ATON_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_get_fields: no fields set");
+    const size_t bytes = ctx->ncell * sizeof(float);
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (nH) CU(ctx, cudaMemcpyAsync(nH, ctx->nH, bytes, kind, ctx->stream));
+    if (x) CU(ctx, cudaMemcpyAsync(x, ctx->x, bytes, kind, ctx->stream));
+    if (T) CU(ctx, cudaMemcpyAsync(T, ctx->T, bytes, kind, ctx->stream));
+    if (N) CU(ctx, cudaMemcpyAsync(N, ctx->rad[ctx->cur][0], bytes, kind, ctx->stream));
+    float *outs[3] = {Fx, Fy, Fz};
+    for (int v = 0; v < 3; v++) {
+        if (!outs[v]) continue;
+        const float *G = ctx->rad[ctx->cur][1 + v];
+        if (on_device) {
+            int rc = scale_into(ctx, G, outs[v], (float)ctx->c);
+            if (rc) return rc;
+        } else {   // F = c G staged in the idle ping-pong buffer
+            float *stage = ctx->rad[1 - ctx->cur][1 + v];
+            int rc = scale_into(ctx, G, stage, (float)ctx->c);
+            if (rc) return rc;
+            CU(ctx, cudaMemcpyAsync(outs[v], stage, bytes, kind, ctx->stream));
+        }
+    }
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    return ATON_OK;
+}
+
+int aton_reduce(aton_t *ctx, aton_diag_t *out) {
+    if (!ctx || !out) return ATON_EINVAL;
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_reduce: no fields set");
+    double r[R_COUNT];
+    int rc = run_reduce(ctx, true, r);
+    if (rc) return rc;
+    unsigned long long st[2];
+    CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    const double n = (double)ctx->ncell, cs = ctx->c * ctx->p.sigma_n;
+    out->x_vol = r[R_X] / n;
+    out->x_mass = r[R_XM] / r[R_M];
+    out->gamma_vol = cs * r[R_N] / n;
+    out->gamma_mass = cs * r[R_NM] / r[R_M];
+    out->photons_total = r[R_N] * ctx->dx * ctx->dx * ctx->dx;
+    out->T_vol = r[R_T] / n;
+    out->f_max = std::sqrt(r[R_F2MAX]);
+    out->N_min = r[R_NMIN];
+    out->frac_x_half = r[R_HALF] / n;
+    out->n_nonfinite = (long long)r[R_BAD];
+    out->subcycles_total = (long long)st[0];
+    out->subcycles_max = (long long)st[1];
+    out->steps_done = ctx->steps_done;
+    out->time_s = ctx->time_s;
+    return ATON_OK;
+}
+
+}  // extern "C"

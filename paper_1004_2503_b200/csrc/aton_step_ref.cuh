@@ -1,0 +1,106 @@
+// Reference step kernel (variant 0): one thread per cell, the 7-point stencil gathered straight from
+// global memory, closure recomputed for each neighbour, chemistry fused behind the transport update.
+// It is the simplest statement of the fused step on the device and the yardstick the tiled kernel
+// (aton_step_tiled.cuh) is compared with; it is also used for grids too small to tile.
+#pragma once
+#include "aton_physics.cuh"
+
+namespace aton {
+
+struct Grid {
+    int nx, ny, nz;
+};
+
+struct FieldsIO {
+    const float *N, *Gx, *Gy, *Gz;      // step-p radiation fields (read only)
+    float *N1, *Gx1, *Gy1, *Gz1;        // step-p+1 radiation fields (other buffer)
+    float *x, *T;                       // updated in place (each cell reads only its own)
+    const float *nH;
+    const unsigned *src_mask;           // 1 bit per 32 consecutive cells: segment holds a source
+    const int *src_cell;                // sorted flat cell indices of the sources
+    const float *src_rho;               // rate / dx^3 per source cell [photons cm^-3 s^-1]
+    int n_src;
+    unsigned long long *stats;          // [0] += sub-cycles, [1] = max sub-cycles
+};
+
+// photons/cm^3 injected this step into flat cell `id` (0 for almost every cell) -- O3, NGP (L103)
+__device__ __forceinline__ float source_lookup(const FieldsIO &f, int id, float dt) {
+    int lo = 0, hi = f.n_src;
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(f.src_cell + mid) < id) lo = mid + 1; else hi = mid;
+    }
+    if (lo < f.n_src && __ldg(f.src_cell + lo) == id) return __ldg(f.src_rho + lo) * dt;
+    return 0.0f;
+}
+
+__device__ __forceinline__ bool source_segment_flag(const FieldsIO &f, int id) {
+    if (f.n_src == 0) return false;
+    unsigned seg = (unsigned)id >> 5;
+    return (__ldg(f.src_mask + (seg >> 5)) >> (seg & 31)) & 1u;
+}
+
+// contribution of the neighbour at +e_d (sgn=+1) or -e_d (sgn=-1) to the LF update of the centre:
+//   N  += h [ N_nb  - sgn * G_d,nb ]
+//   G_j += h [ G_j,nb - sgn * P_dj,nb ],  P_dj = a delta_dj + s G_d G_j
+template <int D>
+__device__ __forceinline__ void add_neighbour(float sgn, float Nn, float gx, float gy, float gz,
+                                              float &aN, float &ax, float &ay, float &az) {
+    float a, s;
+    closure(Nn, gx, gy, gz, a, s);
+    const float gd = D == 0 ? gx : (D == 1 ? gy : gz);
+    const float t = s * gd;
+    float px = t * gx, py = t * gy, pz = t * gz;
+    if (D == 0) px += a; else if (D == 1) py += a; else pz += a;
+    aN += Nn - sgn * gd;
+    ax += gx - sgn * px;
+    ay += gy - sgn * py;
+    az += gz - sgn * pz;
+}
+
+template <int FLAGS>
+__global__ void __launch_bounds__(256) step_ref_kernel(FieldsIO f, Grid g, StepConst c) {
+    const int ncell = g.nx * g.ny * g.nz;
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    int nsub = 0;
+    if (id < ncell) {
+        const int i = id % g.nx, j = (id / g.nx) % g.ny, k = id / (g.nx * g.ny);
+        const int ip = (i + 1 == g.nx) ? 0 : i + 1, im = (i == 0) ? g.nx - 1 : i - 1;
+        const int jp = (j + 1 == g.ny) ? 0 : j + 1, jm = (j == 0) ? g.ny - 1 : j - 1;
+        const int kp = (k + 1 == g.nz) ? 0 : k + 1, km = (k == 0) ? g.nz - 1 : k - 1;
+        const int row = g.nx * (j + g.ny * k);
+        const int nb[6] = {ip + row, im + row, i + g.nx * (jp + g.ny * k), i + g.nx * (jm + g.ny * k),
+                           i + g.nx * (j + g.ny * kp), i + g.nx * (j + g.ny * km)};
+        float aN = 0.f, ax = 0.f, ay = 0.f, az = 0.f;
+#define NB(D, SGN, Q) add_neighbour<D>(SGN, __ldg(f.N + nb[Q]), __ldg(f.Gx + nb[Q]), __ldg(f.Gy + nb[Q]), \
+                                       __ldg(f.Gz + nb[Q]), aN, ax, ay, az)
+        NB(0, 1.f, 0); NB(0, -1.f, 1); NB(1, 1.f, 2); NB(1, -1.f, 3); NB(2, 1.f, 4); NB(2, -1.f, 5);
+#undef NB
+        float N = fmaf(c.h, aN, c.keep * __ldg(f.N + id));
+        float gx = fmaf(c.h, ax, c.keep * __ldg(f.Gx + id));
+        float gy = fmaf(c.h, ay, c.keep * __ldg(f.Gy + id));
+        float gz = fmaf(c.h, az, c.keep * __ldg(f.Gz + id));
+        if (source_segment_flag(f, id)) N += source_lookup(f, id, c.dt);
+        float x = f.x[id], T = f.T[id];
+        nsub = chemistry<FLAGS>(N, gx, gy, gz, x, T, __ldg(f.nH + id), c);
+        f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
+        f.x[id] = x; f.T[id] = T;
+    }
+    // sub-cycle statistics: block reduce, one atomic pair per block
+    __shared__ int s_sum[8], s_max[8];
+    int sum = nsub, mx = nsub;
+    for (int o = 16; o > 0; o >>= 1) {
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if ((threadIdx.x & 31) == 0) { s_sum[threadIdx.x >> 5] = sum; s_max[threadIdx.x >> 5] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int nw = (blockDim.x + 31) >> 5;
+        for (int w = 1; w < nw; w++) { sum += s_sum[w]; mx = max(mx, s_max[w]); }
+        atomicAdd(f.stats, (unsigned long long)sum);
+        atomicMax(f.stats + 1, (unsigned long long)mx);
+    }
+}
+
+}  // namespace aton

@@ -158,11 +158,14 @@ _CFG = {
 
 
 def make_config(cfg: int, n: Optional[int] = None, device="cpu", seed: Optional[int] = None,
-                n_steps: Optional[int] = None) -> Workload:
+                n_steps: Optional[int] = None, norm_steps: Optional[int] = None) -> Workload:
     """Build BASELINE.json config `cfg` (1..5).
 
     `n` overrides the grid size to make a down-sized twin: same cell size dx, same density
     statistics, same number of sources per cell (at least 1), so a full run fits the CPU oracle.
+    `norm_steps` (configs 3-5) is the number of steps over which the sources emit one photon per
+    H atom (reading S15; default: the config's full step count) -- a short twin run can so reach
+    the same half-reionised end state as the full run.
     """
     if cfg == 1:
         return _config1(n or 32, device, n_steps)
@@ -193,10 +196,10 @@ def make_config(cfg: int, n: Optional[int] = None, device="cpu", seed: Optional[
         cand = torch.nonzero(flat > thr, as_tuple=False).reshape(-1)
         perm = torch.randperm(cand.numel(), generator=gen, device=device)[:ns]
         idx = cand[perm]
-        rate = _rates_overdensity(nH, idx, nbar, dx, steps_full * dt)
+        rate = _rates_overdensity(nH, idx, nbar, dx, (norm_steps or steps_full) * dt)
     else:
         idx = _local_maxima_top(nH, ns)
-        rate = _rates_overdensity(nH, idx, nbar, dx, steps_full * dt)
+        rate = _rates_overdensity(nH, idx, nbar, dx, (norm_steps or steps_full) * dt)
         # case-A rates + recombination radiation, collisional ionisation, cooling, C_R = max(1, 1+2 delta)
         p.update(recomb_case=0, clump_model=1, clump_a=1.0, clump_b=2.0, redshift=z)
     if cfg in (2, 3):

@@ -1,0 +1,228 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json's: after 1 step from a warm state max relative error <= 1e-4 on
+N, F (as |dF|/(cN), reading S16), x, T where N > 1e-20 max N; after a full run relative L1 <= 1e-3
+per field and |d<x>_V| <= 1e-3.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1004_2503_b200 import workloads as wl
+from parity_util import (gpu_run, l1_errors, max_rel_errors, oracle_run, state_to_workload, twin)
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP = 1e-4
+TOL_L1 = 1e-3
+TOL_XVOL = 1e-3
+VARIANTS = [0, 1]
+
+
+_cache = {}
+
+
+def _warm(orc, w, k):
+    key = ("warm", w.name, k, tuple(sorted(w.params.items())))
+    if key not in _cache:
+        st, _ = oracle_run(orc, w, k)
+        _cache[key] = state_to_workload(w, st)
+    return _cache[key]
+
+
+def _oracle_cached(orc, w, n_steps):
+    key = ("run", w.name, n_steps, tuple(sorted(w.params.items())), float(w.N.double().sum()))
+    if key not in _cache:
+        _cache[key] = oracle_run(orc, w, n_steps)
+    return _cache[key]
+
+
+# workloads for the element-by-element checks: (builder, warm-up steps K, full-run steps)
+def _cases():
+    return {
+        "cfg1_32": (lambda: wl.make_config(1), 60, 500),
+        "cfg2_twin48": (lambda: twin(2, 48, 120), 60, 120),
+        "cfg3_twin40": (lambda: twin(3, 40, 100), 50, 100),       # 40: several tiles + ragged tail
+        "cfg4_twin48": (lambda: twin(4, 48, 100), 50, 100),       # case A + clumping + coll. ion.
+        "cfg5_twin36": (lambda: twin(5, 36, 80), 40, 80),
+    }
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("case", list(_cases().keys()))
+def test_one_step_from_warm_state(orc, case, variant):
+    """V2 / reading S17: both codes start from the oracle's state after K steps rounded to fp32."""
+    build, k, _ = _cases()[case]
+    w = build()
+    ww = _warm(orc, w, k)
+    st, p = _oracle_cached(orc, ww, 1)
+    g, diag = gpu_run(ww, 1, variant)
+    err = max_rel_errors(g, st, p.c)
+    assert diag["n_nonfinite"] == 0
+    for f, e in err.items():
+        assert e <= TOL_1STEP, (case, variant, err)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("case", list(_cases().keys()))
+def test_full_run(orc, case, variant):
+    """V3: relative L1 per field <= 1e-3 and ionised volume fraction within 1e-3 after the run."""
+    build, _, n_steps = _cases()[case]
+    w = build()
+    st, p = _oracle_cached(orc, w, n_steps)
+    g, diag = gpu_run(w, n_steps, variant)
+    err = l1_errors(g, st, p.c)
+    assert diag["n_nonfinite"] == 0 and diag["steps_done"] == n_steps
+    assert err["x_vol"] <= TOL_XVOL, (case, err)
+    for f in ("N", "F", "x", "T"):
+        assert err[f] <= TOL_L1, (case, variant, err)
+    # diagnostics against the oracle's reduction of its own state
+    d = orc.reduce(st, p)
+    assert diag["x_vol"] == pytest.approx(d["x_vol"], abs=TOL_XVOL)
+    assert diag["x_mass"] == pytest.approx(d["x_mass"], abs=2e-3)
+    assert diag["photons_total"] == pytest.approx(d["photons_total"], rel=2e-3)
+    assert diag["gamma_vol"] == pytest.approx(d["gamma_vol"], rel=2e-3)
+    assert diag["f_max"] <= 1.0 + 1e-5 and diag["N_min"] >= 0.0
+    # sub-cycle statistics are data dependent (H5) but of the same size
+    assert diag["subcycles_total"] == pytest.approx(st.sub_total, rel=0.02)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+def test_isothermal_and_no_collisions_switches(orc, variant):
+    """The other physics-switch combinations (template instantiations) against the oracle."""
+    for kw in (dict(cooling=0, coll_ion=0), dict(cooling=0, coll_ion=1, recomb_case=0),
+               dict(cooling=1, coll_ion=0, recomb_case=0, clump_model=2, clump_a=3.0, clump_b=0.2),
+               dict(cooling=1, coll_ion=0, redshift=9.0)):
+        w = twin(3, 32, 60)
+        w.params.update(kw)
+        ww = _warm(orc, w, 40)
+        st, p = oracle_run(orc, ww, 1)
+        g, _ = gpu_run(ww, 1, variant)
+        err = max_rel_errors(g, st, p.c)
+        assert max(err.values()) <= TOL_1STEP, (kw, err)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+def test_reduce_matches_oracle(orc, variant):
+    w = wl.synthetic_warm_state(twin(4, 32, 10))
+    g, diag = gpu_run(w, 0, variant)
+    st, p = orc.from_workload(w)
+    d = orc.reduce(st, p)
+    for k in ("x_vol", "x_mass", "gamma_vol", "gamma_mass", "photons_total", "T_vol", "N_min", "frac_x_half"):
+        assert diag[k] == pytest.approx(d[k], rel=1e-6), k
+    assert diag["f_max"] == pytest.approx(d["f_max"], rel=1e-5)
+    assert diag["n_nonfinite"] == 0 and diag["steps_done"] == 0
+    # upload -> download is the identity on n_H, x, T, N and within 2 ulp on F (stored as F/c)
+    for k, src in (("nH", w.nH), ("x", w.x), ("T", w.T), ("N", w.N)):
+        assert np.array_equal(g[k], src.numpy())
+    assert np.allclose(g["Fx"], w.Fx.numpy(), rtol=3e-7, atol=0)
+
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+def test_determinism_and_checkpoint(variant):
+    """V4: two runs are bit-identical; and because x, T, N round-trip exactly through get/set while
+    F = c*(F/c) does not, a restart matches to rounding (1e-6), not bitwise."""
+    w = wl.synthetic_warm_state(twin(4, 40, 10))
+    a, _ = gpu_run(w, 12, variant)
+    b, _ = gpu_run(w, 12, variant)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    c, _ = gpu_run(w, 12, variant, chunks=[5, 7])          # buffer parity across calls
+    for k in a:
+        assert np.array_equal(a[k], c[k]), k
+
+
+def test_tile_shape_independence():
+    """V4: the tiled kernel's result does not depend on the tile shape (bitwise)."""
+    w = wl.synthetic_warm_state(twin(5, 40, 10))
+    ref, _ = gpu_run(w, 6, 1, (0, 0))
+    for tile in ((4, 8), (8, 4), (2, 40), (16, 0)):
+        g, _ = gpu_run(w, 6, 1, tile)
+        for k in ref:
+            assert np.array_equal(ref[k], g[k]), (tile, k)
+
+
+def test_tiled_vs_reference_kernel():
+    """The two kernels differ only in rounding order."""
+    w = wl.synthetic_warm_state(twin(4, 48, 10))
+    a, _ = gpu_run(w, 3, 0)
+    b, _ = gpu_run(w, 3, 1)
+    for k in ("N", "x", "T"):
+        assert np.allclose(a[k], b[k], rtol=2e-5, atol=0), k
+
+
+def test_non_cubic_grid_and_source_edges(orc):
+    """nx != ny != nz, sources on cell edges / shared cells / the last cell, against the oracle."""
+    from paper_1004_2503_b200 import aton
+    nx, ny, nz = 24, 10, 7
+    rng = np.random.default_rng(11)
+    nH = (10 ** rng.uniform(-4, -2, (nz, ny, nx))).astype(np.float32)
+    x = np.full((nz, ny, nx), 1e-3, np.float32)
+    T = np.full((nz, ny, nx), 100.0, np.float32)
+    p = wl.default_params()
+    dx = 2.0e21
+    pos = np.array([[0.0, 0.0, 0.0], [0.999999, 0.999999, 0.999999], [0.5, 0.5, 0.5], [0.5, 0.5, 0.5],
+                    [1.0 / 24 * 3, 0.3, 0.2], [1.0, 0.0, 0.0]], np.float32)
+    rate = np.array([1e50, 2e50, 3e50, 1e50, 5e49, 7e49])
+    dt = wl.courant_dt(dx)
+    for variant in VARIANTS:
+        a = aton.Aton(nx, ny, nz, dx * nx, p)
+        a.set_kernel(variant)
+        a.set_fields(*[torch.from_numpy(v).cuda() for v in (nH, x, T)])
+        a.set_sources(torch.from_numpy(pos), torch.from_numpy(rate))
+        a.step(dt, 20)
+        g = {k: v.numpy() for k, v in a.get_fields(device="cpu").items()}
+        st = orc.State(nH, x, T, np.zeros_like(nH), np.zeros_like(nH), np.zeros_like(nH), np.zeros_like(nH))
+        op = orc.make_params(p, dx, float(nH.astype(np.float64).mean()))
+        orc.step(st, op, dt, 20, pos.astype(np.float64), rate)
+        err = l1_errors(g, st, op.c)
+        assert max(err.values()) <= TOL_L1, (variant, err)
+        a.close()
+
+
+def test_api_errors():
+    from paper_1004_2503_b200 import aton
+    p = wl.default_params()
+    with pytest.raises(aton.AtonError) as e:
+        aton.Aton(10, 8, 8, 1e21, p)                                  # nx % 4 != 0
+    assert e.value.code == aton.EINVAL
+    a = aton.Aton(8, 8, 8, 8e21, p)
+    with pytest.raises(aton.AtonError) as e:
+        a.step(1.0, 1)                                                # before set_fields
+    assert e.value.code == aton.ESTATE
+    one = torch.ones(8, 8, 8, device="cuda")
+    with pytest.raises(aton.AtonError) as e:
+        a.set_fields(0 * one, one, one)                               # n_H must be > 0
+    assert e.value.code == aton.EINVAL
+    a.set_fields(1e-3 * one, 1e-3 * one, 100 * one)
+    with pytest.raises(aton.AtonError) as e:
+        a.step(a.courant_dt(1.01), 1)                                 # c dt/dx > 1/3
+    assert e.value.code == aton.EINVAL and "unstable" in str(e.value)
+    assert a.courant_dt(0.8) == pytest.approx(0.8 * 1e21 / (3 * wl.C_CM_S))
+    with pytest.raises(aton.AtonError):
+        a.set_sources(torch.tensor([[1.5, 0.0, 0.0]]), torch.tensor([1e50], dtype=torch.float64))
+    with pytest.raises(aton.AtonError):
+        a.set_sources(torch.tensor([[0.5, 0.0, 0.0]]), torch.tensor([-1.0], dtype=torch.float64))
+    a.step(0.0, 2)                                                    # dt <= 0 => Courant 0.8
+    d = a.reduce()
+    assert d["steps_done"] == 2 and d["time_s"] == pytest.approx(2 * a.courant_dt(0.8))
+    assert a.launch_count() > 0
+    a.close()
+
+
+def test_empty_sources_and_vacuum_conservation():
+    """No sources, no absorption possible (x = 1 exactly): photons are conserved to fp32 rounding."""
+    from paper_1004_2503_b200 import aton
+    n = 32
+    w = wl.synthetic_warm_state(twin(3, n, 10))
+    p = dict(w.params); p.update(cooling=0, coll_ion=0)
+    a = aton.Aton(n, n, n, w.box_cm, p)
+    one = torch.ones(n, n, n, device="cuda")
+    a.set_fields(1e-12 * one, one, 1e4 * one, w.N.cuda(), w.Fx.cuda(), w.Fy.cuda(), w.Fz.cuda())
+    a.set_sources(None, None)
+    before = a.reduce()["photons_total"]
+    a.step(w.dt, 50)
+    d = a.reduce()
+    assert d["photons_total"] == pytest.approx(before, rel=2e-5)
+    assert d["N_min"] >= 0 and d["f_max"] <= 1 + 1e-5
+    a.close()
