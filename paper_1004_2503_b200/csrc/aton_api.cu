@@ -48,7 +48,7 @@ struct aton_ctx {
     bool have_fields = false;
     long long steps_done = 0, launches = 0;
     double time_s = 0;
-    int variant = 0, tile_y = 0, tile_z = 0;
+    int variant = 1, tile_y = 0, tile_z = 0;
     char err[512] = "";
 };
 
