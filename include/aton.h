@@ -74,11 +74,14 @@ typedef struct {
     long long n_nonfinite;        /* cells holding a NaN/Inf in any of N, F, x, T */
     long long subcycles_total;    /* chemistry sub-cycles summed over cells and steps since aton_set_fields */
     long long subcycles_max;      /* largest per-cell, per-step sub-cycle count seen */
+    long long cells_subcycled;    /* cell-steps that needed more than one sub-cycle and were redone by the
+                                     fix-up kernel (kernel variant 2 only; 0 otherwise) */
     long long steps_done;         /* steps since aton_set_fields */
     double time_s;                /* sum of dt since aton_set_fields */
 } aton_diag_t;
 
-/* Create a context: allocates 11 float32 device arrays of nx*ny*nz (7 fields + 4 ping-pong).
+/* Create a context: allocates 11 float32 device arrays of nx*ny*nz (7 fields + 4 ping-pong) and one bit
+ * per cell of work flags.
  * `stream` is borrowed for the life of the context.  On failure *out is NULL. */
 int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box,
               const aton_params_t *params, void *cuda_stream);
@@ -112,8 +115,9 @@ int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float 
 int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
 /* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
- * memory); 1 = tiled streaming kernel (default).  tile_y / tile_z choose the tile shape of
- * variant 1 (0 = default); results do not depend on the tile shape. */
+ * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel
+ * (default).  tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows,
+ * tile_z = planes per z-chunk); results do not depend on the tile shape.  ATON_EINVAL otherwise. */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */

@@ -43,7 +43,8 @@ class Diag(C.Structure):
                 ("gamma_mass", C.c_double), ("photons_total", C.c_double), ("T_vol", C.c_double),
                 ("f_max", C.c_double), ("N_min", C.c_double), ("frac_x_half", C.c_double),
                 ("n_nonfinite", C.c_longlong), ("subcycles_total", C.c_longlong),
-                ("subcycles_max", C.c_longlong), ("steps_done", C.c_longlong), ("time_s", C.c_double)]
+                ("subcycles_max", C.c_longlong), ("cells_subcycled", C.c_longlong),
+                ("steps_done", C.c_longlong), ("time_s", C.c_double)]
 
 
 class AtonError(RuntimeError):

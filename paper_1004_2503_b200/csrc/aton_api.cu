@@ -17,6 +17,7 @@
 #include "aton_reduce.cuh"
 #include "aton_step_ref.cuh"
 #include "aton_step_tiled.cuh"
+#include "aton_step_fused.cuh"
 
 using namespace aton;
 
@@ -42,13 +43,15 @@ struct aton_ctx {
     int *src_cell = nullptr;
     float *src_rho = nullptr;
     int n_src = 0;
-    unsigned long long *stats = nullptr;   // device [2]
+    unsigned long long *stats = nullptr;   // device [3]
+    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variant 2)
+    long long fast_subcycles = 0;          // variant 2: one sub-cycle per cell and step, counted on the host
     double *partials = nullptr;            // device [REDUCE_BLOCKS+1][R_COUNT]
     double nH_mean = 1.0;
     bool have_fields = false;
     long long steps_done = 0, launches = 0;
     double time_s = 0;
-    int variant = 1, tile_y = 0, tile_z = 0;
+    int variant = 2, tile_y = 0, tile_z = 0;
     char err[512] = "";
 };
 
@@ -90,6 +93,7 @@ StepConst make_step_const(const aton_ctx *ctx, double dt) {
     s.zff0 = (float)(1.42e-27 / kb15);
     s.zexc0 = (float)(7.5e-19 / kb15);
     s.l2_zci0 = (float)std::log2(E0_EV * EV_ERG * 21.11 / kb15);
+    s.zci_over_beta = (float)(E0_EV * EV_ERG / kb15);
     const double zp1 = 1.0 + p.redshift;
     s.compton0 = p.redshift >= 0.0 ? (float)(5.65e-36 * zp1 * zp1 * zp1 * zp1 / kb15) : 0.0f;
     s.t_cmb = (float)(2.726 * zp1);
@@ -116,6 +120,7 @@ FieldsIO make_io(const aton_ctx *ctx) {
     f.src_mask = ctx->src_mask; f.src_cell = ctx->src_cell; f.src_rho = ctx->src_rho;
     f.n_src = ctx->n_src;
     f.stats = ctx->stats;
+    f.defer_mask = ctx->defer_mask;
     return f;
 }
 
@@ -127,7 +132,12 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
         step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc);
         return cudaGetLastError();
     }
-    return launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+    if (ctx->variant == 1) return launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+    int launches = 0;
+    const cudaError_t e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream, &launches);
+    ctx->launches += launches - 1;      // launch_step counted one
+    ctx->fast_subcycles += (long long)ctx->ncell;
+    return e;
 }
 
 cudaError_t launch_step(aton_ctx *ctx, const StepConst &sc) {
@@ -211,10 +221,13 @@ int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, cons
     float **slots[11] = {&ctx->rad[0][0], &ctx->rad[0][1], &ctx->rad[0][2], &ctx->rad[0][3], &ctx->rad[1][0],
                          &ctx->rad[1][1], &ctx->rad[1][2], &ctx->rad[1][3], &ctx->x, &ctx->T, &ctx->nH};
     for (int i = 0; i < 11 && e == cudaSuccess; i++) e = cudaMalloc((void **)slots[i], bytes);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, 3 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->partials, sizeof(double) * (REDUCE_BLOCKS + 1) * R_COUNT);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_mask, sizeof(unsigned) * (ctx->ncell / 1024 + 1));
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 2 * sizeof(unsigned long long), ctx->stream);
+    const size_t defer_bytes = sizeof(unsigned) * (ctx->ncell / 32 + 1);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->defer_mask, defer_bytes);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->defer_mask, 0, defer_bytes, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->ncell / 1024 + 1), ctx->stream);
     if (e != cudaSuccess) {
         int code = fail(nullptr, e == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,
@@ -233,7 +246,7 @@ void aton_free(aton_t *ctx) {
         for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
     cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
     cudaFree(ctx->src_mask); cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
-    cudaFree(ctx->stats); cudaFree(ctx->partials);
+    cudaFree(ctx->stats); cudaFree(ctx->partials); cudaFree(ctx->defer_mask);
     delete ctx;
 }
 
@@ -243,8 +256,8 @@ long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0;
 
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
-    if (variant < 0 || variant > 1) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0 or 1");
-    if (variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z))
+    if (variant < 0 || variant > 2) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0, 1 or 2");
+    if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     return ATON_OK;
@@ -275,7 +288,7 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
             }
         }
     }
-    CU(ctx, cudaMemsetAsync(ctx->stats, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    CU(ctx, cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream));
     double red[R_COUNT];
     int rc = run_reduce(ctx, false, red);
     if (rc) return rc;
@@ -283,6 +296,7 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
         return fail(ctx, ATON_EINVAL, "aton_set_fields: n_H must be finite and > 0 everywhere (min %g)", red[R_NHMIN]);
     ctx->nH_mean = red[R_M] / (double)ctx->ncell;
     ctx->steps_done = 0;
+    ctx->fast_subcycles = 0;
     ctx->time_s = 0.0;
     ctx->have_fields = true;
     return ATON_OK;
@@ -404,7 +418,7 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out) {
     double r[R_COUNT];
     int rc = run_reduce(ctx, true, r);
     if (rc) return rc;
-    unsigned long long st[2];
+    unsigned long long st[3];
     CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
     const double n = (double)ctx->ncell, cs = ctx->c * ctx->p.sigma_n;
@@ -418,8 +432,9 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out) {
     out->N_min = r[R_NMIN];
     out->frac_x_half = r[R_HALF] / n;
     out->n_nonfinite = (long long)r[R_BAD];
-    out->subcycles_total = (long long)st[0];
-    out->subcycles_max = (long long)st[1];
+    out->subcycles_total = (long long)st[0] + ctx->fast_subcycles;
+    out->subcycles_max = std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
+    out->cells_subcycled = (long long)st[2];
     out->steps_done = ctx->steps_done;
     out->time_s = ctx->time_s;
     return ATON_OK;

@@ -26,6 +26,7 @@ struct StepConst {        // per aton_step call, host-computed in fp64, passed b
     float l2_zrec0;       // log2( zeta_rec prefactor / (1.5 kB) )  (case A or B)
     float zff0, zexc0;    // prefactors / (1.5 kB)
     float l2_zci0;        // log2( 13.6 eV * 21.11 / (1.5 kB) )
+    float zci_over_beta;  // 13.6 eV / (1.5 kB)  [K]: zeta_ci = 13.6 eV * beta
     float compton0;       // 5.65e-36 (1+z)^4 / (1.5 kB), 0 when off
     float t_cmb;          // 2.726 (1+z)
     float eps_sub;

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 TOL_1STEP = 1e-4
 TOL_L1 = 1e-3
 TOL_XVOL = 1e-3
-VARIANTS = [0, 1]
+VARIANTS = [0, 1, 2]
 
 
 _cache = {}
@@ -48,7 +48,7 @@ def _cases():
     }
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
 @pytest.mark.parametrize("case", list(_cases().keys()))
 def test_one_step_from_warm_state(orc, case, variant):
     """V2 / reading S17: both codes start from the oracle's state after K steps rounded to fp32."""
@@ -63,7 +63,7 @@ def test_one_step_from_warm_state(orc, case, variant):
         assert e <= TOL_1STEP, (case, variant, err)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
 @pytest.mark.parametrize("case", list(_cases().keys()))
 def test_full_run(orc, case, variant):
     """V3: relative L1 per field <= 1e-3 and ionised volume fraction within 1e-3 after the run."""
@@ -87,7 +87,7 @@ def test_full_run(orc, case, variant):
     assert diag["subcycles_total"] == pytest.approx(st.sub_total, rel=0.02)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
 def test_isothermal_and_no_collisions_switches(orc, variant):
     """The other physics-switch combinations (template instantiations) against the oracle."""
     for kw in (dict(cooling=0, coll_ion=0), dict(cooling=0, coll_ion=1, recomb_case=0),
@@ -102,7 +102,7 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
         assert max(err.values()) <= TOL_1STEP, (kw, err)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
 def test_reduce_matches_oracle(orc, variant):
     w = wl.synthetic_warm_state(twin(4, 32, 10))
     g, diag = gpu_run(w, 0, variant)
@@ -118,7 +118,7 @@ def test_reduce_matches_oracle(orc, variant):
     assert np.allclose(g["Fx"], w.Fx.numpy(), rtol=3e-7, atol=0)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
 def test_determinism_and_checkpoint(variant):
     """V4: two runs are bit-identical; and because x, T, N round-trip exactly through get/set while
     F = c*(F/c) does not, a restart matches to rounding (1e-6), not bitwise."""
@@ -132,23 +132,43 @@ def test_determinism_and_checkpoint(variant):
         assert np.array_equal(a[k], c[k]), k
 
 
-def test_tile_shape_independence():
-    """V4: the tiled kernel's result does not depend on the tile shape (bitwise)."""
+@pytest.mark.parametrize("variant,tiles", [(1, ((4, 8), (8, 4), (2, 40), (16, 0))),
+                                           (2, ((6, 0), (14, 0), (8, 5), (6, 40), (14, 1)))], ids=["v1", "v2"])
+def test_tile_shape_independence(variant, tiles):
+    """V4: the tiled kernels' result does not depend on the tile shape (bitwise)."""
     w = wl.synthetic_warm_state(twin(5, 40, 10))
-    ref, _ = gpu_run(w, 6, 1, (0, 0))
-    for tile in ((4, 8), (8, 4), (2, 40), (16, 0)):
-        g, _ = gpu_run(w, 6, 1, tile)
+    ref, dref = gpu_run(w, 6, variant, (0, 0))
+    for tile in tiles:
+        g, d = gpu_run(w, 6, variant, tile)
         for k in ref:
             assert np.array_equal(ref[k], g[k]), (tile, k)
+        assert d["subcycles_total"] == dref["subcycles_total"] and d["cells_subcycled"] == dref["cells_subcycled"]
 
 
 def test_tiled_vs_reference_kernel():
-    """The two kernels differ only in rounding order."""
+    """The three kernels differ only in rounding order (and, for variant 2, in which cells take the
+    sub-cycled path when the 10 % rule is decided within rounding: H5, continuous in the result)."""
     w = wl.synthetic_warm_state(twin(4, 48, 10))
-    a, _ = gpu_run(w, 3, 0)
-    b, _ = gpu_run(w, 3, 1)
-    for k in ("N", "x", "T"):
-        assert np.allclose(a[k], b[k], rtol=2e-5, atol=0), k
+    a, da = gpu_run(w, 3, 0)
+    for variant in (1, 2):
+        b, db = gpu_run(w, 3, variant)
+        for k in ("N", "x", "T"):
+            assert np.allclose(a[k], b[k], rtol=5e-5, atol=0), (variant, k)
+        assert db["subcycles_total"] == pytest.approx(da["subcycles_total"], rel=1e-3)
+        assert db["subcycles_max"] == da["subcycles_max"]
+
+
+def test_fixup_path_statistics():
+    """Variant 2: cells that need sub-cycling are redone by the fix-up kernel, counted, and the mask is
+    left clean (a second identical context gives the same counts; an isothermal run never defers)."""
+    w = wl.make_config(1)
+    g, d = gpu_run(w, 40, 2)
+    assert d["cells_subcycled"] > 0 and d["subcycles_max"] > 1
+    assert d["subcycles_total"] > 40 * w.n ** 3
+    w2 = wl.make_config(1)
+    w2.params.update(cooling=0)
+    g2, d2 = gpu_run(w2, 10, 2)
+    assert d2["cells_subcycled"] == 0 and d2["subcycles_max"] == 1 and d2["subcycles_total"] == 10 * w.n ** 3
 
 
 def test_non_cubic_grid_and_source_edges(orc):
