@@ -116,12 +116,20 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
 /* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
  * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel
- * (default).  tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows,
+ * (default).  tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6,
  * tile_z = planes per z-chunk); results do not depend on the tile shape.  ATON_EINVAL otherwise. */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */
 long long aton_launch_count(const aton_t *ctx);
+
+/* Measurement aid (bench.py's roofline): with on != 0 every later aton_step brackets the dominant
+ * kernel of each step (the fused transport + injection + chemistry kernel; not the sub-cycle fix-up)
+ * with CUDA events on the context's stream.  Calling it again (on or off) discards the events. */
+int aton_set_timing(aton_t *ctx, int on);
+
+/* Sum [ms] and number of the bracketed launches since aton_set_timing(ctx, 1).  Synchronises. */
+int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches);
 
 void aton_free(aton_t *ctx);
 

@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libaton.so")
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt", "aton_step",
-           "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_free",
-           "aton_last_error")
+           "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_set_timing",
+           "aton_kernel_time", "aton_free", "aton_last_error")
 
 
 class Grid(C.Structure):
@@ -85,6 +85,10 @@ def load_library(path: Optional[str] = None):
     L.aton_set_kernel.argtypes = [vp, C.c_int, C.c_int, C.c_int]
     L.aton_launch_count.restype = C.c_longlong
     L.aton_launch_count.argtypes = [vp]
+    L.aton_set_timing.restype = C.c_int
+    L.aton_set_timing.argtypes = [vp, C.c_int]
+    L.aton_kernel_time.restype = C.c_int
+    L.aton_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.aton_free.restype = None
     L.aton_free.argtypes = [vp]
     L.aton_last_error.restype = C.c_char_p
@@ -185,6 +189,15 @@ class Aton:
 
     def set_kernel(self, variant: int, tile_y: int = 0, tile_z: int = 0):
         self._check(self._L.aton_set_kernel(self._h, variant, tile_y, tile_z))
+
+    def set_timing(self, on: bool):
+        self._check(self._L.aton_set_timing(self._h, int(bool(on))))
+
+    def kernel_time(self):
+        """(sum of ms, launches) of the event-bracketed dominant step kernel since set_timing(True)."""
+        ms, n = C.c_double(), C.c_longlong()
+        self._check(self._L.aton_kernel_time(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def launch_count(self) -> int:
         return int(self._L.aton_launch_count(self._h))

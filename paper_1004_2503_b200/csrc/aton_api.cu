@@ -52,6 +52,8 @@ struct aton_ctx {
     long long steps_done = 0, launches = 0;
     double time_s = 0;
     int variant = 2, tile_y = 0, tile_z = 0;
+    bool timing = false;                   // aton_set_timing: CUDA events around the dominant step kernel
+    std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch
     char err[512] = "";
 };
 
@@ -124,19 +126,38 @@ FieldsIO make_io(const aton_ctx *ctx) {
     return f;
 }
 
+// aton_set_timing: an event right before / after the dominant kernel of a step
+void time_mark(aton_ctx *ctx) {
+    if (!ctx->timing) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, ctx->stream);
+    ctx->ev.push_back(e);
+}
+
 template <int FLAGS>
 cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
     if (ctx->variant == 0) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((ctx->ncell + threads - 1) / threads);
+        time_mark(ctx);
         step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc);
+        time_mark(ctx);
         return cudaGetLastError();
     }
-    if (ctx->variant == 1) return launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
-    int launches = 0;
-    const cudaError_t e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream, &launches);
-    ctx->launches += launches - 1;      // launch_step counted one
+    if (ctx->variant == 1) {
+        time_mark(ctx);
+        const cudaError_t e = launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+        time_mark(ctx);
+        return e;
+    }
+    time_mark(ctx);
+    cudaError_t e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+    time_mark(ctx);
     ctx->fast_subcycles += (long long)ctx->ncell;
+    if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
+    e = launch_step_fixup<FLAGS>(f, ctx->g, sc, ctx->stream);   // only cooling can sub-cycle
+    ctx->launches++;
     return e;
 }
 
@@ -242,6 +263,7 @@ int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, cons
 
 void aton_free(aton_t *ctx) {
     if (!ctx) return;
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (int b = 0; b < 2; b++)
         for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
     cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
@@ -260,6 +282,28 @@ int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
+    return ATON_OK;
+}
+
+int aton_set_timing(aton_t *ctx, int on) {
+    if (!ctx) return ATON_EINVAL;
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    ctx->ev.clear();
+    ctx->timing = on != 0;
+    return ATON_OK;
+}
+
+int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches) {
+    if (!ctx || !ms_total || !n_launches) return ATON_EINVAL;
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    for (size_t i = 0; i + 1 < ctx->ev.size(); i += 2) {
+        float ms = 0.0f;
+        CU(ctx, cudaEventElapsedTime(&ms, ctx->ev[i], ctx->ev[i + 1]));
+        tot += ms;
+    }
+    *ms_total = tot;
+    *n_launches = (long long)(ctx->ev.size() / 2);
     return ATON_OK;
 }
 

@@ -353,22 +353,22 @@ inline bool fused_shape_ok(int tile_y, int tile_z) {
     return (tile_y == 0 || tile_y == 6 || tile_y == 8 || tile_y == 14) && tile_z >= 0;
 }
 
-// one step = fused kernel (+ fix-up when the physics can sub-cycle, i.e. cooling is on)
+// one step = fused kernel, then (when the physics can sub-cycle, i.e. cooling is on) the fix-up kernel
 template <int FLAGS>
 cudaError_t launch_step_fused(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_y, int tile_z,
-                              cudaStream_t stream, int *launches) {
-    cudaError_t e;
-    if (tile_y == 6) e = launch_step_fused_ty<FLAGS, 6>(f, g, c, tile_z, stream);
-    else if (tile_y == 14) e = launch_step_fused_ty<FLAGS, 14>(f, g, c, tile_z, stream);
-    else e = launch_step_fused_ty<FLAGS, 8>(f, g, c, tile_z, stream);
-    *launches = 1;
-    if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
+                              cudaStream_t stream) {
+    if (tile_y == 8) return launch_step_fused_ty<FLAGS, 8>(f, g, c, tile_z, stream);
+    if (tile_y == 14) return launch_step_fused_ty<FLAGS, 14>(f, g, c, tile_z, stream);
+    return launch_step_fused_ty<FLAGS, 6>(f, g, c, tile_z, stream);    // default: measured fastest
+}
+
+template <int FLAGS>
+cudaError_t launch_step_fixup(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream) {
     const long ncell = (long)g.nx * g.ny * g.nz;
     const int nwords = (int)((ncell + 31) / 32);
     const int nchunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
     const int blocks = nchunks < 148 * 8 ? nchunks : 148 * 8;
     step_fixup_kernel<FLAGS><<<blocks, FIXUP_THREADS, 0, stream>>>(f, c, nwords);
-    *launches = 2;
     return cudaGetLastError();
 }
 
