@@ -115,9 +115,12 @@ int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float 
 int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
 /* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
- * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel
- * (default).  tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6,
- * tile_z = planes per z-chunk); results do not depend on the tile shape.  ATON_EINVAL otherwise. */
+ * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel;
+ * 3 (default) = variant 2's arithmetic with full tiles, no halo warps and a split-phase barrier -- used
+ * when nx % 128 == 0 and ny % tile_y == 0, otherwise the variant-2 kernel runs.  tile_y / tile_z choose
+ * the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6; variant 3: tile_y in
+ * {4, 8, 16}, default 8; tile_z = planes per z-chunk); results do not depend on the variant (2 vs 3) or
+ * the tile shape.  ATON_EINVAL otherwise. */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */

@@ -18,6 +18,7 @@
 #include "aton_step_ref.cuh"
 #include "aton_step_tiled.cuh"
 #include "aton_step_fused.cuh"
+#include "aton_step_v3.cuh"
 
 using namespace aton;
 
@@ -51,7 +52,7 @@ struct aton_ctx {
     bool have_fields = false;
     long long steps_done = 0, launches = 0;
     double time_s = 0;
-    int variant = 2, tile_y = 0, tile_z = 0;
+    int variant = 3, tile_y = 0, tile_z = 0;
     bool timing = false;                   // aton_set_timing: CUDA events around the dominant step kernel
     std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch
     char err[512] = "";
@@ -151,8 +152,12 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
         time_mark(ctx);
         return e;
     }
+    // variant 3 needs full tiles (nx % 128 == 0, ny % TY == 0); other grids run the variant-2 kernel
+    const int ty3 = ctx->variant == 3 ? v3_pick_ty(ctx->g, ctx->tile_y) : 0;
     time_mark(ctx);
-    cudaError_t e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+    cudaError_t e = ty3 ? launch_step_v3<FLAGS>(f, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
+                        : launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 3 ? 0 : ctx->tile_y,
+                                                   ctx->variant == 3 ? 0 : ctx->tile_z, ctx->stream);
     time_mark(ctx);
     ctx->fast_subcycles += (long long)ctx->ncell;
     if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
@@ -278,8 +283,9 @@ long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0;
 
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
-    if (variant < 0 || variant > 2) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0, 1 or 2");
-    if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)))
+    if (variant < 0 || variant > 3) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0..3");
+    if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)) ||
+        (variant == 3 && !v3_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     return ATON_OK;

@@ -246,3 +246,82 @@ def test_empty_sources_and_vacuum_conservation():
     assert d["photons_total"] == pytest.approx(before, rel=2e-5)
     assert d["N_min"] >= 0 and d["f_max"] <= 1 + 1e-5
     a.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# Variant 3 (full-tile kernel: nx % 128 == 0, ny % tile_y == 0).  The cubic twins above are too small
+# for it (they run the variant-2 kernel under the default variant), so it gets non-cubic grids whose
+# x extent spans one or two 128-cell tiles, several y tiles and a ragged z chunk.
+# ------------------------------------------------------------------------------------------------
+def _slab_case(nx, ny, nz, flags7, seed):
+    """Random log-normal-ish density on an (nz, ny, nx) grid, sources on tile corners / edges, physics of
+    config 4 (flags7: case A + recombination radiation + clumping) or config 2 (case B)."""
+    rng = np.random.default_rng(seed)
+    nH = (2e-4 * np.exp(1.5 * rng.standard_normal((nz, ny, nx)) - 1.125)).astype(np.float32)
+    x = np.full((nz, ny, nx), 1e-3, np.float32)
+    T = np.full((nz, ny, nx), 100.0, np.float32)
+    p = wl.default_params()
+    p.update(redshift=8.0)
+    if flags7:
+        p.update(recomb_case=0, clump_model=1, clump_a=1.0, clump_b=2.0)
+    dx = 3.0e21
+    cells = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (127, 7, 1), (128 % nx, 8 % ny, 2 % nz), (nx // 2, ny // 2, nz // 2),
+             (3, ny - 1, 0), (nx - 4, 0, nz - 1)]
+    pos = np.array([[(i + 0.5) / nx, (j + 0.5) / ny, (k + 0.5) / nz] for i, j, k in cells], np.float32)
+    rate = 10 ** rng.uniform(49.5, 51, len(cells))
+    return nH, x, T, p, dx, pos, rate
+
+
+def _run_slab(variant, tile, nH, x, T, p, dx, pos, rate, n_steps, rad=None):
+    from paper_1004_2503_b200 import aton
+    nz, ny, nx = nH.shape
+    a = aton.Aton(nx, ny, nz, dx * nx, p)
+    a.set_kernel(variant, *tile)
+    f = [torch.from_numpy(np.ascontiguousarray(v, dtype=np.float32)).cuda() for v in (nH, x, T) + tuple(rad or ())]
+    a.set_fields(*f)
+    a.set_sources(torch.from_numpy(pos), torch.from_numpy(rate))
+    a.step(wl.courant_dt(dx), n_steps)
+    g = {k: v.numpy() for k, v in a.get_fields(device="cpu").items()}
+    d = a.reduce()
+    a.close()
+    return g, d
+
+
+@pytest.mark.parametrize("shape,flags7", [((128, 16, 11), True), ((256, 24, 9), False), ((128, 8, 3), True)],
+                         ids=["128x16x11_A", "256x24x9_B", "128x8x3_A"])
+def test_v3_full_tile_kernel_against_oracle(orc, shape, flags7):
+    nx, ny, nz = shape
+    nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, flags7, seed=nx + ny + nz)
+    dt = wl.courant_dt(dx)
+    op = orc.make_params(p, dx, float(nH.astype(np.float64).mean()))
+    zero = np.zeros_like(nH)
+    # full run from the dark start (V3 metric)
+    st = orc.State(nH, x, T, zero, zero, zero, zero)
+    orc.step(st, op, dt, 40, pos.astype(np.float64), rate)
+    g, d = _run_slab(3, (0, 0), nH, x, T, p, dx, pos, rate, 40)
+    err = l1_errors(g, st, op.c)
+    assert d["n_nonfinite"] == 0 and max(err.values()) <= TOL_L1, err
+    # one step from the oracle's warm state rounded to fp32 (V2 metric)
+    warm = [np.ascontiguousarray(v, dtype=np.float32) for v in (st.x, st.T, st.N, st.Fx, st.Fy, st.Fz)]
+    st1 = orc.State(nH, *warm)
+    orc.step(st1, op, dt, 1, pos.astype(np.float64), rate)
+    for tile in ((0, 0), (4, 2), (8, 5)) + (((16, 0),) if ny % 16 == 0 else ()):
+        g1, d1 = _run_slab(3, tile, nH, warm[0], warm[1], p, dx, pos, rate, 1, rad=warm[2:])
+        e1 = max_rel_errors(g1, st1, op.c)
+        assert max(e1.values()) <= TOL_1STEP, (tile, e1)
+
+
+def test_v3_tile_shape_independence_determinism_and_v2_agreement():
+    nH, x, T, p, dx, pos, rate = _slab_case(256, 32, 13, True, seed=5)
+    ref, dref = _run_slab(3, (0, 0), nH, x, T, p, dx, pos, rate, 25)
+    assert dref["cells_subcycled"] > 0
+    for tile in ((0, 0), (4, 0), (16, 0), (8, 3), (16, 13), (4, 1)):
+        g, d = _run_slab(3, tile, nH, x, T, p, dx, pos, rate, 25)
+        for k in ref:
+            assert np.array_equal(ref[k], g[k]), (tile, k)
+        assert d["subcycles_total"] == dref["subcycles_total"] and d["cells_subcycled"] == dref["cells_subcycled"]
+    # variant 2 sums the x and y neighbour terms in another order: equal to rounding
+    g2, d2 = _run_slab(2, (0, 0), nH, x, T, p, dx, pos, rate, 25)
+    for k in ("N", "x", "T"):
+        assert np.allclose(ref[k], g2[k], rtol=5e-5, atol=0), k
+    assert d2["subcycles_total"] == pytest.approx(dref["subcycles_total"], rel=1e-3)
