@@ -74,8 +74,8 @@ typedef struct {
     long long n_nonfinite;        /* cells holding a NaN/Inf in any of N, F, x, T */
     long long subcycles_total;    /* chemistry sub-cycles summed over cells and steps since aton_set_fields */
     long long subcycles_max;      /* largest per-cell, per-step sub-cycle count seen */
-    long long cells_subcycled;    /* cell-steps that needed more than one sub-cycle and were redone by the
-                                     fix-up kernel (kernel variant 2 only; 0 otherwise) */
+    long long cells_subcycled;    /* cell-steps handed to the fix-up kernel: cells that needed more than one
+                                     sub-cycle (variants 2-4) and, for variant 4, the source cells */
     long long steps_done;         /* steps since aton_set_fields */
     double time_s;                /* sum of dt since aton_set_fields */
 } aton_diag_t;
@@ -116,11 +116,12 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
 /* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
  * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel;
- * 3 (default) = variant 2's arithmetic with full tiles, no halo warps and a split-phase barrier -- used
- * when nx % 128 == 0 and ny % tile_y == 0, otherwise the variant-2 kernel runs.  tile_y / tile_z choose
- * the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6; variant 3: tile_y in
- * {4, 8, 16}, default 8; tile_z = planes per z-chunk); results do not depend on the variant (2 vs 3) or
- * the tile shape.  ATON_EINVAL otherwise. */
+ * 3 = variant 2's arithmetic with full CTA tiles and a split-phase barrier (nx % 128 == 0, ny % tile_y == 0);
+ * 4 (default) = warp-autonomous tiles, no inter-warp synchronisation, sources injected by the fix-up
+ * kernel (nx % 32 == 0, ny % 4 == 0).  A grid a variant cannot tile runs the variant-2 kernel.
+ * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6;
+ * variant 3: tile_y in {4, 8, 16}, default 8; variant 4: tile_y must be 0; tile_z = planes per z-chunk);
+ * results agree between variants to rounding and do not depend on the tile shape.  ATON_EINVAL otherwise. */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */

@@ -19,6 +19,7 @@
 #include "aton_step_tiled.cuh"
 #include "aton_step_fused.cuh"
 #include "aton_step_v3.cuh"
+#include "aton_step_v4.cuh"
 
 using namespace aton;
 
@@ -45,14 +46,15 @@ struct aton_ctx {
     float *src_rho = nullptr;
     int n_src = 0;
     unsigned long long *stats = nullptr;   // device [3]
-    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variant 2)
+    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variants 2-4)
+    unsigned *src_bits = nullptr;          // device, 1 bit per cell: the cell holds a source (variant 4)
     long long fast_subcycles = 0;          // variant 2: one sub-cycle per cell and step, counted on the host
     double *partials = nullptr;            // device [REDUCE_BLOCKS+1][R_COUNT]
     double nH_mean = 1.0;
     bool have_fields = false;
     long long steps_done = 0, launches = 0;
     double time_s = 0;
-    int variant = 3, tile_y = 0, tile_z = 0;
+    int variant = 4, tile_y = 0, tile_z = 0;
     bool timing = false;                   // aton_set_timing: CUDA events around the dominant step kernel
     std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch
     char err[512] = "";
@@ -124,6 +126,8 @@ FieldsIO make_io(const aton_ctx *ctx) {
     f.n_src = ctx->n_src;
     f.stats = ctx->stats;
     f.defer_mask = ctx->defer_mask;
+    f.src_bits = ctx->src_bits;
+    f.fix_inject = 0;
     return f;
 }
 
@@ -152,16 +156,22 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
         time_mark(ctx);
         return e;
     }
-    // variant 3 needs full tiles (nx % 128 == 0, ny % TY == 0); other grids run the variant-2 kernel
+    // variant 4 needs nx % 32 == 0, ny % 4 == 0; variant 3 nx % 128 == 0, ny % TY == 0; other grids run the
+    // variant-2 kernel.  Only variant 4 leaves the source injection to the fix-up kernel.
+    const bool use4 = ctx->variant == 4 && v4_grid_ok(ctx->g);
     const int ty3 = ctx->variant == 3 ? v3_pick_ty(ctx->g, ctx->tile_y) : 0;
+    FieldsIO f2 = f;
+    f2.fix_inject = use4 ? 1 : 0;
     time_mark(ctx);
-    cudaError_t e = ty3 ? launch_step_v3<FLAGS>(f, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
-                        : launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 3 ? 0 : ctx->tile_y,
-                                                   ctx->variant == 3 ? 0 : ctx->tile_z, ctx->stream);
+    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, ctx->tile_z, ctx->stream)
+                    : ty3 ? launch_step_v3<FLAGS>(f2, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
+                          : launch_step_fused<FLAGS>(f2, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0,
+                                                     ctx->variant == 2 ? ctx->tile_z : 0, ctx->stream);
     time_mark(ctx);
     ctx->fast_subcycles += (long long)ctx->ncell;
-    if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
-    e = launch_step_fixup<FLAGS>(f, ctx->g, sc, ctx->stream);   // only cooling can sub-cycle
+    // the fix-up runs when cells can sub-cycle (cooling on) or, for variant 4, when there are sources
+    if (e != cudaSuccess || !((FLAGS & F_COOL) || (use4 && ctx->n_src > 0))) return e;
+    e = launch_step_fixup<FLAGS>(f2, ctx->g, sc, ctx->stream);
     ctx->launches++;
     return e;
 }
@@ -253,6 +263,8 @@ int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, cons
     const size_t defer_bytes = sizeof(unsigned) * (ctx->ncell / 32 + 1);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->defer_mask, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->defer_mask, 0, defer_bytes, ctx->stream);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_bits, defer_bytes);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_bits, 0, defer_bytes, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->ncell / 1024 + 1), ctx->stream);
     if (e != cudaSuccess) {
@@ -273,7 +285,7 @@ void aton_free(aton_t *ctx) {
         for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
     cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
     cudaFree(ctx->src_mask); cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
-    cudaFree(ctx->stats); cudaFree(ctx->partials); cudaFree(ctx->defer_mask);
+    cudaFree(ctx->stats); cudaFree(ctx->partials); cudaFree(ctx->defer_mask); cudaFree(ctx->src_bits);
     delete ctx;
 }
 
@@ -283,9 +295,9 @@ long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0;
 
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
-    if (variant < 0 || variant > 3) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0..3");
+    if (variant < 0 || variant > 4) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0..4");
     if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)) ||
-        (variant == 3 && !v3_shape_ok(tile_y, tile_z)))
+        (variant == 3 && !v3_shape_ok(tile_y, tile_z)) || (variant == 4 && (tile_y != 0 || tile_z < 0)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     return ATON_OK;
@@ -400,11 +412,15 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
     cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
     ctx->src_cell = nullptr; ctx->src_rho = nullptr; ctx->n_src = 0;
     CU(ctx, cudaMemcpyAsync(ctx->src_mask, mask.data(), sizeof(unsigned) * nwords, cudaMemcpyHostToDevice, ctx->stream));
+    CU(ctx, cudaMemsetAsync(ctx->src_bits, 0, sizeof(unsigned) * (ctx->ncell / 32 + 1), ctx->stream));
     if (nu > 0) {
         CU(ctx, cudaMalloc((void **)&ctx->src_cell, sizeof(int) * nu));
         CU(ctx, cudaMalloc((void **)&ctx->src_rho, sizeof(float) * nu));
         CU(ctx, cudaMemcpyAsync(ctx->src_cell, ucell.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, ctx->stream));
         CU(ctx, cudaMemcpyAsync(ctx->src_rho, rho.data(), sizeof(float) * nu, cudaMemcpyHostToDevice, ctx->stream));
+        source_bits_kernel<<<(unsigned)((nu + 255) / 256), 256, 0, ctx->stream>>>(ctx->src_cell, (int)nu, ctx->src_bits);
+        ctx->launches++;
+        CU(ctx, cudaGetLastError());
     }
     CU(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->n_src = (int)nu;

@@ -108,10 +108,11 @@ __device__ __forceinline__ f2 clumping2(f2 nH, const StepConst &c) {
 
 // ---------------------------------------------------------------- O4, one sub-step of length dt
 // In/out: N, G (after transport + injection), x, T.  Returns a 2-bit mask: bit h set = half h needs
-// sub-cycling (its values are returned unchanged).
+// sub-cycling (its values are returned unchanged).  `force`: halves to leave unchanged and report
+// whatever the 10 % rule says (variant 4 hands its source cells to the fix-up kernel this way).
 template <int FLAGS>
 __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2 &x, f2 &T, f2 nH,
-                                               const StepConst &c) {
+                                               const StepConst &c, unsigned force = 0u) {
     constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL;
     const bool warm = fmaxf(lo(T), hi(T)) > 1100.0f;
     Rates2 r;
@@ -121,13 +122,13 @@ __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2
     const f2 ne = x * nH;
     const f2 theta = fma2(x, T, T);                                      // (1 + x) T
     const f2 crz = fma2(CR, r.zrec, r.zff);
-    unsigned defer = 0;
+    unsigned defer = force;
     if (COOL) {
         // estimated net heating rate / (1.5 kB nH) [K/s]: the Anninos 10 % rule decides on sub-cycling
         const f2 lamK = fma2(nH, (x * x) * crz + (x * y) * r.zxy, (x * c.compton0) * (T - c.t_cmb));
         const f2 ed = abs2(fma2(y * N, c.heat_rate_K, splat(0.0f) - lamK));
         const f2 lhs = ed * c.dt, rhs = theta * c.eps_sub;
-        defer = (lo(lhs) > lo(rhs) ? 1u : 0u) | (hi(lhs) > hi(rhs) ? 2u : 0u);
+        defer |= (lo(lhs) > lo(rhs) ? 1u : 0u) | (hi(lhs) > hi(rhs) ? 2u : 0u);
     }
     // backward-Euler coupled (N, x) update, solved for delta = x' - x
     const float dt = c.dt;
@@ -167,9 +168,7 @@ __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2
         Tn = max2(thn * rcp2(xn + 1.0f), 1.0f);
     }
     const f2 Nn = nH * Pa, gxn = gx * att, gyn = gy * att, gzn = gz * att;
-    if (defer == 0) {       // common case: both halves done
-        N = Nn; gx = gxn; gy = gyn; gz = gzn; x = xn; T = Tn;
-    } else {
+    {   // branch-free: a deferred half keeps its input values
         const bool k0 = defer & 1u, k1 = defer & 2u;
 #define ATON_KEEP(old, nw) old = pk(k0 ? lo(old) : lo(nw), k1 ? hi(old) : hi(nw))
         ATON_KEEP(N, Nn); ATON_KEEP(gx, gxn); ATON_KEEP(gy, gyn); ATON_KEEP(gz, gzn);

@@ -112,4 +112,10 @@ __global__ void __launch_bounds__(256) scale_kernel(const float4 *__restrict__ i
     }
 }
 
+// one bit per cell holding a source (variant 4's per-cell source flags); cells are unique
+__global__ void __launch_bounds__(256) source_bits_kernel(const int *__restrict__ cells, int n, unsigned *bits) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) atomicOr(bits + ((unsigned)cells[s] >> 5), 1u << (cells[s] & 31));
+}
+
 }  // namespace aton

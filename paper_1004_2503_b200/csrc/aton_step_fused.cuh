@@ -300,6 +300,7 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(FieldsIO f, S
                 const int id = queue[it];
                 float N = f.N1[id], gx = f.Gx1[id], gy = f.Gy1[id], gz = f.Gz1[id];
                 float x = f.x[id], T = f.T[id];
+                if (f.fix_inject && source_segment_flag(f, id)) N += source_lookup(f, id, c.dt);
                 const int ns = chemistry<FLAGS>(N, gx, gy, gz, x, T, __ldg(f.nH + id), c);
                 f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
                 f.x[id] = x; f.T[id] = T;

@@ -21,7 +21,9 @@ struct FieldsIO {
     const float *src_rho;               // rate / dx^3 per source cell [photons cm^-3 s^-1]
     int n_src;
     unsigned long long *stats;          // [0] += sub-cycles, [1] = max sub-cycles, [2] += cells redone by the fix-up
-    unsigned *defer_mask;               // variant 2: 1 bit per cell, set = needs sub-cycling (fix-up kernel clears it)
+    unsigned *defer_mask;               // variant 2+: 1 bit per cell, set = needs sub-cycling (fix-up kernel clears it)
+    const unsigned *src_bits;           // variant 4: 1 bit per cell, set = the cell holds a source
+    int fix_inject;                     // variant 4: the fix-up kernel injects the sources (the step kernel did not)
 };
 
 // photons/cm^3 injected this step into flat cell `id` (0 for almost every cell) -- O3, NGP (L103)

@@ -38,16 +38,23 @@ __device__ __forceinline__ void mbar_init(unsigned addr, unsigned count) {
 __device__ __forceinline__ void mbar_arrive(unsigned addr) {
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned addr, unsigned parity) {
+__device__ __forceinline__ bool mbar_try(unsigned addr, unsigned parity) {
+    unsigned ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "ATON_WAIT:\n"
-        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra ATON_DONE;\n"
-        "bra ATON_WAIT;\n"
-        "ATON_DONE:\n"
-        "}\n" ::"r"(addr), "r"(parity) : "memory");
+        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    return ok != 0;
+}
+#ifndef ATON_WAIT_SLEEP_NS
+#define ATON_WAIT_SLEEP_NS 0
+#endif
+__device__ __forceinline__ void mbar_wait(unsigned addr, unsigned parity) {
+    while (!mbar_try(addr, parity)) {
+        if (ATON_WAIT_SLEEP_NS > 0) __nanosleep(ATON_WAIT_SLEEP_NS);
+    }
 }
 
 template <int FLAGS, int TY>

@@ -1,0 +1,303 @@
+// Fused step kernel, variant 4 (the product kernel for grids with nx % 32 == 0 and ny % 4 == 0):
+// WARP-AUTONOMOUS tiles.  Transport + one chemistry sub-step in one pass over HBM (52 B per cell-update);
+// source cells and cells that need sub-cycling go to step_fixup_kernel.
+//
+// Why: profiles/r01_c_step_v3_512.md -- in variant 3 every warp spends 20 % of its time spinning on the
+// per-plane CTA barrier (the slowest of 8 warps, its DRAM latency hiccups and the two edge warps' extra
+// halo row set the pace), 9 % on the source-mask load and 3 % in source binary searches, at 4 warps per
+// scheduler with nothing else to issue.  Here no warp ever waits for another warp:
+//  * a warp owns a tile of 32 x-cells x 4 rows (lane = row r = lane>>3, quad q = lane&7) and marches
+//    through a z-chunk; x neighbours come from shuffles inside the row's 8 lanes, y neighbours through a
+//    4 KB warp-private shared-memory patch fenced by __syncwarp, z neighbours stay in registers;
+//  * the tile's own halo (the rows below / above, the cells left / right) is staged and closed by the warp
+//    itself in one extra pass (lanes of rows 0 and 3 take the y halo rows, lanes q = 0 / 7 the x halo
+//    cells): ~10 % more instructions and 1.6x more L2->SM traffic on (N, G) for zero synchronisation;
+//    HBM traffic is unchanged (the re-reads hit L2: neighbouring tiles run at the same time);
+//  * the z loop is peeled (first two / last iteration) so the steady-state body is one straight-line
+//    block: no `if (in plane)`, `if (finished)`, no divergent halo branches (predicated stores instead),
+//    no source lookups -- the scheduler interleaves the chemistry's MUFU chains with the transport FMAs;
+//  * per-cell source flags come from a 1-bit-per-cell mask: a source cell is treated like a cell that
+//    needs sub-cycling (chemistry result discarded, flagged); the fix-up kernel injects and sub-cycles.
+// Arithmetic per cell is variant 3's (same order of operations): results are bit-identical to variant 3
+// except in source cells (scalar instead of packed chemistry there).
+#pragma once
+#include <type_traits>
+
+#include "aton_step_v3.cuh"
+
+namespace aton {
+
+struct V4Cfg {
+    static constexpr int WX = 32, WY = 4;                // cells per warp tile
+    static constexpr int RS = 40;                        // raw row: quads at col 4 + 4q, x halos at 3 and 36
+    static constexpr int RAW_FIELD = (WY + 2) * RS;      // row slots 0 / WY+1 = y halo rows
+    static constexpr int RAW_BUF = 4 * RAW_FIELD;        // [field][slot][RS]
+    static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
+    static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][32]
+    static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN;
+    static constexpr int WARPS = 4, THREADS = 32 * WARPS;
+    static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
+};
+
+template <int FLAGS>
+__global__ void __launch_bounds__(V4Cfg::THREADS, 4)
+step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
+    using C = V4Cfg;
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int r = lane >> 3, q = lane & 7;
+    const int xt = blockIdx.x * C::WARPS + warp;         // x tile of this warp
+    if (xt * C::WX >= g.nx) return;                      // ragged last CTA in x: warps are independent
+    float *raw = smem + warp * C::WARP_FLOATS;           // [2][4][6][RS], thread-private entries
+    float *wyp = raw + 2 * C::RAW_BUF;                   // [4][4][32] plus terms
+    float *wym = wyp + C::W_SIGN;                        //            minus terms
+
+    const int x0 = xt * C::WX, y0 = blockIdx.y * C::WY, z0 = blockIdx.z * lz;
+    const int lzn = min(lz, g.nz - z0);
+    const int plane = g.nx * g.ny;
+    const int rowoff = (y0 + r) * g.nx + x0 + 4 * q;     // own quad inside a plane
+    // y halo row of this lane: rows 0 / 3 take the row below / above the tile (others: a harmless re-read)
+    const bool hbot = r == 0, htop = r == C::WY - 1;
+    const int jh = hbot ? (y0 == 0 ? g.ny - 1 : y0 - 1) : (htop ? (y0 + C::WY == g.ny ? 0 : y0 + C::WY) : y0 + r);
+    const int hoff = jh * g.nx + x0 + 4 * q;
+    const int hslot = hbot ? 0 : (htop ? C::WY + 1 : r + 1);
+    // x halo cell of this lane: q = 0 the cell left of the tile, q = 7 the cell right of it
+    const bool edge_l = q == 0, edge_r = q == 7;
+    const int xh = edge_l ? (x0 == 0 ? g.nx - 1 : x0 - 1) : (x0 + C::WX == g.nx ? 0 : x0 + C::WX);
+    const int xoff = (y0 + r) * g.nx + xh;
+    const int my = (r + 1) * C::RS + 4 + 4 * q;          // own quad inside a raw field
+    const int myh = hslot * C::RS + 4 + 4 * q;           // halo-row quad
+    const int mxh = (r + 1) * C::RS + (edge_l ? 3 : 36); // x halo cell (valid for edge lanes)
+    const float *src[4] = {f.N, f.Gx, f.Gy, f.Gz};
+
+    int kst = z0 == 0 ? g.nz - 1 : z0 - 1;               // plane index staged next (periodic)
+    auto stage = [&](int m, bool inpl) {
+        float *dst = raw + (m & 1) * C::RAW_BUF;
+        const int base = kst * plane;
+#pragma unroll
+        for (int v = 0; v < 4; v++) cp_async16(dst + v * C::RAW_FIELD + my, src[v] + base + rowoff);
+        if (inpl) {
+            if (hbot || htop) {
+#pragma unroll
+                for (int v = 0; v < 4; v++) cp_async16(dst + v * C::RAW_FIELD + myh, src[v] + base + hoff);
+            }
+            if (edge_l || edge_r) {
+#pragma unroll
+                for (int v = 0; v < 4; v++) cp_async4(dst + v * C::RAW_FIELD + mxh, src[v] + base + xoff);
+            }
+        }
+        cp_async_commit();
+        kst = kst + 1 == g.nz ? 0 : kst + 1;
+    };
+
+    const f2 zero = splat(0.0f);
+    Quad pend, zup;          // plane m-1 awaiting its +z term; h*(U + F_z) of plane m-1
+#pragma unroll
+    for (int p = 0; p < 2; p++)
+#pragma unroll
+        for (int v = 0; v < 4; v++) { pend.v[p][v] = zero; zup.v[p][v] = zero; }
+
+    int kcur = z0 == 0 ? g.nz - 1 : z0 - 1;
+    int ocur = kcur * plane + rowoff;    // flat index of this thread's quad in plane m
+    int oprev = 0;                       //                                  in plane m-1
+    int m = 0;
+
+    // one z iteration; INPL: plane m belongs to the chunk (x / y terms needed); FIN: plane m-1 is finished here
+    auto iter = [&](auto inpl_tag, auto fin_tag, bool stage_next, bool next_inpl) {
+        constexpr bool INPL = decltype(inpl_tag)::value, FIN = decltype(fin_tag)::value;
+        cp_async_wait_all();                             // this thread's part of plane m has landed
+        const float *buf = raw + (m & 1) * C::RAW_BUF;
+        if (stage_next) stage(m + 1, next_inpl);
+
+        // early loads for the chemistry of plane m-1
+        float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), T4 = x4, h4 = make_float4(1.f, 1.f, 1.f, 1.f);
+        unsigned srcw = 0;
+        if (FIN) {
+            x4 = *reinterpret_cast<const float4 *>(f.x + oprev);
+            T4 = *reinterpret_cast<const float4 *>(f.T + oprev);
+            h4 = __ldg(reinterpret_cast<const float4 *>(f.nH + oprev));
+            srcw = __ldg(f.src_bits + ((unsigned)oprev >> 5));
+        }
+        // ---- closure of the staged quad
+        Quad u;
+        f2 a[2], s[2];
+        {
+            const float4 n4 = *reinterpret_cast<const float4 *>(buf + my);
+            const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + my);
+            const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + my);
+            const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + my);
+#pragma unroll
+            for (int p = 0; p < 2; p++) {
+                u.v[p][0] = ld_pair(n4, p); u.v[p][1] = ld_pair(gx4, p);
+                u.v[p][2] = ld_pair(gy4, p); u.v[p][3] = ld_pair(gz4, p);
+                closure2(u.v[p][0], u.v[p][1], u.v[p][2], u.v[p][3], a[p], s[p]);
+            }
+        }
+        Quad t;
+        if (INPL) {
+            __syncwarp();                                // every lane has consumed the previous plane's y terms
+            // ---- y: publish (U + F_y) for the row above, (U - F_y) for the row below
+            {
+                f2 F[2][4];
+                flux_row(1, u.v[0], a[0], s[0], F[0]);
+                flux_row(1, u.v[1], a[1], s[1], F[1]);
+#pragma unroll
+                for (int v = 0; v < 4; v++) {
+                    const f2 p0 = u.v[0][v] + F[0][v], p1 = u.v[1][v] + F[1][v];
+                    const f2 m0 = u.v[0][v] - F[0][v], m1 = u.v[1][v] - F[1][v];
+                    if (!htop)
+                        *reinterpret_cast<float4 *>(wyp + v * C::W_COMP + (r + 1) * 32 + 4 * q) =
+                            make_float4(lo(p0), hi(p0), lo(p1), hi(p1));
+                    if (!hbot)
+                        *reinterpret_cast<float4 *>(wym + v * C::W_COMP + (r - 1) * 32 + 4 * q) =
+                            make_float4(lo(m0), hi(m0), lo(m1), hi(m1));
+                }
+            }
+            // ---- the tile's y halo rows (lanes of rows 0 and 3; the others compute and store nothing new)
+            {
+                const float4 n4 = *reinterpret_cast<const float4 *>(buf + myh);
+                const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + myh);
+                const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + myh);
+                const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + myh);
+                f2 w[2][4];
+#pragma unroll
+                for (int p = 0; p < 2; p++) {
+                    f2 e[4] = {ld_pair(n4, p), ld_pair(gx4, p), ld_pair(gy4, p), ld_pair(gz4, p)};
+                    f2 ea, es, F[4];
+                    closure2(e[0], e[1], e[2], e[3], ea, es);
+                    flux_row(1, e, ea, es, F);
+                    const f2 sg = splat(hbot ? 1.0f : -1.0f);
+#pragma unroll
+                    for (int v = 0; v < 4; v++) w[p][v] = fma2(F[v], sg, e[v]);
+                }
+                float *wdst = hbot ? wyp + 4 * q : wym + (C::WY - 1) * 32 + 4 * q;
+                if (hbot || htop) {
+#pragma unroll
+                    for (int v = 0; v < 4; v++)
+                        *reinterpret_cast<float4 *>(wdst + v * C::W_COMP) =
+                            make_float4(lo(w[0][v]), hi(w[0][v]), lo(w[1][v]), hi(w[1][v]));
+                }
+            }
+            __syncwarp();                                // y terms of the plane are visible to the warp
+        }
+        // ---- z: complete plane m-1, start plane m, seed plane m+1
+#pragma unroll
+        for (int p = 0; p < 2; p++) {
+            f2 F[4];
+            flux_row(2, u.v[p], a[p], s[p], F);
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+                pend.v[p][v] = fma2(u.v[p][v] - F[v], c.h, pend.v[p][v]);
+                t.v[p][v] = fma2(u.v[p][v], c.keep, zup.v[p][v]);
+                zup.v[p][v] = (u.v[p][v] + F[v]) * c.h;
+            }
+        }
+        // ---- x: (U + F_x) of the cell to the left, (U - F_x) of the cell to the right
+        if (INPL) {
+            f2 Wp[2][4], Wm[2][4];
+#pragma unroll
+            for (int p = 0; p < 2; p++) {
+                f2 F[4];
+                flux_row(0, u.v[p], a[p], s[p], F);
+#pragma unroll
+                for (int v = 0; v < 4; v++) { Wp[p][v] = u.v[p][v] + F[v]; Wm[p][v] = u.v[p][v] - F[v]; }
+            }
+            f2 eWp[4], eWm[4];
+            {   // the x halo cell of the edge lanes (all lanes run it; only q = 0 / 7 use the result)
+                f2 e[4], ea, es, F[4];
+#pragma unroll
+                for (int v = 0; v < 4; v++) e[v] = splat(buf[v * C::RAW_FIELD + mxh]);
+                closure2(e[0], e[1], e[2], e[3], ea, es);
+                flux_row(0, e, ea, es, F);
+#pragma unroll
+                for (int v = 0; v < 4; v++) { eWp[v] = e[v] + F[v]; eWm[v] = e[v] - F[v]; }
+            }
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+                float left = __shfl_up_sync(0xffffffffu, hi(Wp[1][v]), 1);
+                float right = __shfl_down_sync(0xffffffffu, lo(Wm[0][v]), 1);
+                left = edge_l ? lo(eWp[v]) : left;
+                right = edge_r ? lo(eWm[v]) : right;
+                const f2 sx0 = pk(left + hi(Wm[0][v]), lo(Wp[0][v]) + lo(Wm[1][v]));
+                const f2 sx1 = pk(hi(Wp[0][v]) + hi(Wm[1][v]), lo(Wp[1][v]) + right);
+                t.v[0][v] = fma2(sx0, c.h, t.v[0][v]);
+                t.v[1][v] = fma2(sx1, c.h, t.v[1][v]);
+            }
+        }
+        // ---- plane m-1 has all six contributions: one chemistry sub-step, store; source cells and cells
+        //      that need sub-cycling keep their transported (N, G), old (x, T) and are flagged
+        if (FIN) {
+            const unsigned srcn = (srcw >> (oprev & 31)) & 0xFu;
+            f2 xs[2] = {pk(x4.x, x4.y), pk(x4.z, x4.w)}, Ts[2] = {pk(T4.x, T4.y), pk(T4.z, T4.w)};
+            const f2 hs[2] = {pk(h4.x, h4.y), pk(h4.z, h4.w)};
+            unsigned nib = 0;
+#pragma unroll
+            for (int p = 0; p < 2; p++)
+                nib |= chem_fast2<FLAGS>(pend.v[p][0], pend.v[p][1], pend.v[p][2], pend.v[p][3], xs[p], Ts[p], hs[p], c,
+                                         (srcn >> (2 * p)) & 3u)
+                       << (2 * p);
+#define ATON_ST4(ptr, A, B) *reinterpret_cast<float4 *>(ptr + oprev) = make_float4(lo(A), hi(A), lo(B), hi(B))
+            ATON_ST4(f.N1, pend.v[0][0], pend.v[1][0]);
+            ATON_ST4(f.Gx1, pend.v[0][1], pend.v[1][1]);
+            ATON_ST4(f.Gy1, pend.v[0][2], pend.v[1][2]);
+            ATON_ST4(f.Gz1, pend.v[0][3], pend.v[1][3]);
+            ATON_ST4(f.x, xs[0], xs[1]);
+            ATON_ST4(f.T, Ts[0], Ts[1]);
+#undef ATON_ST4
+            if (nib) atomicOr(f.defer_mask + ((unsigned)oprev >> 5), nib << (oprev & 31));
+        }
+        // ---- y terms of plane m, written straight into the carried registers
+        if (INPL) {
+            const int rp = r * 32 + 4 * q;
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+                const float4 yp = *reinterpret_cast<const float4 *>(wyp + v * C::W_COMP + rp);
+                const float4 ym = *reinterpret_cast<const float4 *>(wym + v * C::W_COMP + rp);
+#pragma unroll
+                for (int p = 0; p < 2; p++)
+                    pend.v[p][v] = fma2(ld_pair(yp, p) + ld_pair(ym, p), c.h, t.v[p][v]);
+            }
+        } else {
+            pend = t;
+        }
+        oprev = ocur;
+        kcur = kcur + 1 == g.nz ? 0 : kcur + 1;
+        ocur = kcur * plane + rowoff;
+        m++;
+    };
+
+    const std::true_type yes{};
+    const std::false_type no{};
+    stage(0, false);
+    iter(no, no, true, true);                  // m = 0: z halo plane below the chunk
+    iter(yes, no, true, true);                 // m = 1: first own plane, nothing to finish yet
+    while (m <= lzn) iter(yes, yes, true, true);   // steady state (the last one stages the z halo plane above)
+    iter(no, yes, false, false);               // m = lzn + 1: z halo plane above, finishes plane lzn
+}
+
+inline bool v4_grid_ok(const Grid &g) { return g.nx % V4Cfg::WX == 0 && g.ny % V4Cfg::WY == 0; }
+
+inline int v4_default_lz(const Grid &g, int tile_z) {
+    if (tile_z > 0) return tile_z < g.nz ? tile_z : g.nz;
+    const long tiles_xy = (long)((g.nx / V4Cfg::WX + V4Cfg::WARPS - 1) / V4Cfg::WARPS) * (g.ny / V4Cfg::WY);
+    int lz = 64;      // largest power of two <= 64 that still gives >= 4 waves of 4 CTAs per SM
+    while (lz > 4 && tiles_xy * ((g.nz + lz - 1) / lz) < 16L * 148) lz >>= 1;
+    return lz < g.nz ? lz : g.nz;
+}
+
+template <int FLAGS>
+cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream) {
+    using C = V4Cfg;
+    static bool attr_done = false;     // one per instantiation
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int lz = v4_default_lz(g, tile_z);
+    const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (g.nz + lz - 1) / lz);
+    step_v4_kernel<FLAGS><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz);
+    return cudaGetLastError();
+}
+
+}  // namespace aton

@@ -265,7 +265,7 @@ def _slab_case(nx, ny, nz, flags7, seed):
     if flags7:
         p.update(recomb_case=0, clump_model=1, clump_a=1.0, clump_b=2.0)
     dx = 3.0e21
-    cells = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (127, 7, 1), (128 % nx, 8 % ny, 2 % nz), (nx // 2, ny // 2, nz // 2),
+    cells = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (127 % nx, 7 % ny, 1 % nz), (128 % nx, 8 % ny, 2 % nz), (nx // 2, ny // 2, nz // 2),
              (3, ny - 1, 0), (nx - 4, 0, nz - 1)]
     pos = np.array([[(i + 0.5) / nx, (j + 0.5) / ny, (k + 0.5) / nz] for i, j, k in cells], np.float32)
     rate = 10 ** rng.uniform(49.5, 51, len(cells))
@@ -287,9 +287,13 @@ def _run_slab(variant, tile, nH, x, T, p, dx, pos, rate, n_steps, rad=None):
     return g, d
 
 
-@pytest.mark.parametrize("shape,flags7", [((128, 16, 11), True), ((256, 24, 9), False), ((128, 8, 3), True)],
-                         ids=["128x16x11_A", "256x24x9_B", "128x8x3_A"])
-def test_v3_full_tile_kernel_against_oracle(orc, shape, flags7):
+@pytest.mark.parametrize("variant,shape,flags7",
+                         [(3, (128, 16, 11), True), (3, (256, 24, 9), False), (3, (128, 8, 3), True),
+                          (4, (128, 16, 11), True), (4, (256, 24, 9), False), (4, (32, 8, 5), True),
+                          (4, (160, 12, 1), True), (4, (64, 4, 70), False)],
+                         ids=["v3_128x16x11_A", "v3_256x24x9_B", "v3_128x8x3_A", "v4_128x16x11_A", "v4_256x24x9_B",
+                              "v4_32x8x5_A", "v4_160x12x1_A", "v4_64x4x70_B"])
+def test_full_tile_kernels_against_oracle(orc, variant, shape, flags7):
     nx, ny, nz = shape
     nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, flags7, seed=nx + ny + nz)
     dt = wl.courant_dt(dx)
@@ -298,25 +302,29 @@ def test_v3_full_tile_kernel_against_oracle(orc, shape, flags7):
     # full run from the dark start (V3 metric)
     st = orc.State(nH, x, T, zero, zero, zero, zero)
     orc.step(st, op, dt, 40, pos.astype(np.float64), rate)
-    g, d = _run_slab(3, (0, 0), nH, x, T, p, dx, pos, rate, 40)
+    g, d = _run_slab(variant, (0, 0), nH, x, T, p, dx, pos, rate, 40)
     err = l1_errors(g, st, op.c)
     assert d["n_nonfinite"] == 0 and max(err.values()) <= TOL_L1, err
+    assert d["subcycles_total"] == pytest.approx(st.sub_total, rel=0.02)
     # one step from the oracle's warm state rounded to fp32 (V2 metric)
     warm = [np.ascontiguousarray(v, dtype=np.float32) for v in (st.x, st.T, st.N, st.Fx, st.Fy, st.Fz)]
     st1 = orc.State(nH, *warm)
     orc.step(st1, op, dt, 1, pos.astype(np.float64), rate)
-    for tile in ((0, 0), (4, 2), (8, 5)) + (((16, 0),) if ny % 16 == 0 else ()):
-        g1, d1 = _run_slab(3, tile, nH, warm[0], warm[1], p, dx, pos, rate, 1, rad=warm[2:])
+    tiles = ((0, 0), (4, 2), (8, 5)) + (((16, 0),) if ny % 16 == 0 else ()) if variant == 3 else ((0, 0), (0, 1), (0, 3), (0, 64))
+    for tile in tiles:
+        g1, d1 = _run_slab(variant, tile, nH, warm[0], warm[1], p, dx, pos, rate, 1, rad=warm[2:])
         e1 = max_rel_errors(g1, st1, op.c)
         assert max(e1.values()) <= TOL_1STEP, (tile, e1)
 
 
-def test_v3_tile_shape_independence_determinism_and_v2_agreement():
+@pytest.mark.parametrize("variant,tiles", [(3, ((0, 0), (4, 0), (16, 0), (8, 3), (16, 13), (4, 1))),
+                                           (4, ((0, 0), (0, 1), (0, 2), (0, 5), (0, 13)))], ids=["v3", "v4"])
+def test_full_tile_kernels_tile_shape_independence_determinism_and_v2_agreement(variant, tiles):
     nH, x, T, p, dx, pos, rate = _slab_case(256, 32, 13, True, seed=5)
-    ref, dref = _run_slab(3, (0, 0), nH, x, T, p, dx, pos, rate, 25)
+    ref, dref = _run_slab(variant, (0, 0), nH, x, T, p, dx, pos, rate, 25)
     assert dref["cells_subcycled"] > 0
-    for tile in ((0, 0), (4, 0), (16, 0), (8, 3), (16, 13), (4, 1)):
-        g, d = _run_slab(3, tile, nH, x, T, p, dx, pos, rate, 25)
+    for tile in tiles:
+        g, d = _run_slab(variant, tile, nH, x, T, p, dx, pos, rate, 25)
         for k in ref:
             assert np.array_equal(ref[k], g[k]), (tile, k)
         assert d["subcycles_total"] == dref["subcycles_total"] and d["cells_subcycled"] == dref["cells_subcycled"]
@@ -325,3 +333,15 @@ def test_v3_tile_shape_independence_determinism_and_v2_agreement():
     for k in ("N", "x", "T"):
         assert np.allclose(ref[k], g2[k], rtol=5e-5, atol=0), k
     assert d2["subcycles_total"] == pytest.approx(dref["subcycles_total"], rel=1e-3)
+
+
+def test_v4_equals_v3_bitwise_without_sources():
+    """Variant 4 keeps variant 3's order of operations per cell; only source cells take another path."""
+    nH, x, T, p, dx, pos, rate = _slab_case(128, 16, 9, True, seed=3)
+    w = wl.synthetic_warm_state(twin(4, 128, 1))            # realizable radiation field to cut a slab from
+    rad = [w.x.numpy()[:9, :16, :], w.T.numpy()[:9, :16, :]] + [t.numpy()[:9, :16, :] for t in (w.N, w.Fx, w.Fy, w.Fz)]
+    none = (np.zeros((0, 3), np.float32), np.zeros(0))
+    a, _ = _run_slab(3, (0, 0), nH, rad[0], rad[1], p, dx, *none, 5, rad=rad[2:])
+    b, _ = _run_slab(4, (0, 0), nH, rad[0], rad[1], p, dx, *none, 5, rad=rad[2:])
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
