@@ -181,7 +181,7 @@ def run_ours(args, rank, world, local_rank):
     if args.state == "warm":
         w = wl.synthetic_warm_state(w)
     a = aton.from_workload(w)
-    variant = 3 if args.variant is None else args.variant
+    variant = 4 if args.variant is None else args.variant
     a.set_kernel(variant, args.tile_y, args.tile_z)
     cells = float(n) ** 3
     stream = torch.cuda.current_stream()
@@ -245,7 +245,7 @@ def run_ours(args, rank, world, local_rank):
     achieved = BYTES_PER_CELL_UPDATE * cells / (kernel_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": recorded_traffic(n),
-                "kernel": {0: "step_ref_kernel", 1: "step_tiled_kernel", 2: "step_fused_kernel", 3: "step_v3_kernel"}[variant],
+                "kernel": {0: "step_ref_kernel", 1: "step_tiled_kernel", 2: "step_fused_kernel", 3: "step_v3_kernel", 4: "step_v4_kernel"}[variant],
                 "kernel_ms": kernel_ms, "kernel_launches_timed": k_n,
                 "kernel_share_of_step": kernel_ms / (ms_total / args.steps), "algorithmic_bytes_per_launch": BYTES_PER_CELL_UPDATE * cells,
                 "peak_source": peak_src}
@@ -283,8 +283,8 @@ def main():
     ap.add_argument("--tile-z", type=int, default=0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--cpu-sample-n", type=int, default=96)
-    ap.add_argument("--cpu-sample-steps", type=int, default=40)
+    ap.add_argument("--cpu-sample-n", type=int, default=128)
+    ap.add_argument("--cpu-sample-steps", type=int, default=100)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

@@ -20,11 +20,13 @@ __device__ __forceinline__ f2 splat(float s) { return pk(s, s); }
 __device__ __forceinline__ float lo(f2 a) {
     float x, y;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v));
+    (void)y;
     return x;
 }
 __device__ __forceinline__ float hi(f2 a) {
     float x, y;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v));
+    (void)x;
     return y;
 }
 __device__ __forceinline__ f2 operator+(f2 a, f2 b) {

@@ -39,8 +39,11 @@ struct V4Cfg {
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
 };
 
+#ifndef ATON_V4_MINB
+#define ATON_V4_MINB 4
+#endif
 template <int FLAGS>
-__global__ void __launch_bounds__(V4Cfg::THREADS, 4)
+__global__ void __launch_bounds__(V4Cfg::THREADS, ATON_V4_MINB)
 step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
     using C = V4Cfg;
     extern __shared__ __align__(16) float smem[];
