@@ -345,3 +345,77 @@ def test_v4_equals_v3_bitwise_without_sources():
     b, _ = _run_slab(4, (0, 0), nH, rad[0], rad[1], p, dx, *none, 5, rad=rad[2:])
     for k in a:
         assert np.array_equal(a[k], b[k]), k
+
+
+# ------------------------------------------------------------------------------------------------
+# BASELINE.json's full size (config 5, 1024^3) in the launch configuration bench.py times (default
+# kernel variant and tile shape).  The oracle cannot run 2^30 cells, but the scheme's domain of
+# dependence is one cell per step: a (m + 2p)^3 sub-cube of the INPUT state advanced p steps by the
+# oracle (with whatever boundary) is exact in its inner m^3, which is compared with the same cells of
+# the full-grid GPU run.  Both codes start from generator output only (dark start, or
+# workloads.synthetic_warm_state): no oracle input comes from the CUDA path.
+# ------------------------------------------------------------------------------------------------
+def _subcube_check(orc, w, state_name, origins, m, p_steps, nH_mean):
+    from paper_1004_2503_b200 import aton
+    n, size = w.n, m + 2 * p_steps
+    a = aton.from_workload(w)
+    a.step(w.dt, p_steps)
+    out = a.get_fields(device="cuda", names=("x", "T", "N", "Fx", "Fy", "Fz"))
+    diag = a.reduce()
+    a.close()
+    assert diag["n_nonfinite"] == 0 and diag["steps_done"] == p_steps
+    src_cell = torch.floor(w.src_pos.double() * n).long() % n           # (ns, 3) as (i, j, k)
+    worst = {}
+    for org in origins:
+        cut = {k: wl.cut_subcube(getattr(w, k), org, size).numpy() for k in ("nH", "x", "T", "N", "Fx", "Fy", "Fz")}
+        st = orc.State(*[cut[k] for k in ("nH", "x", "T", "N", "Fx", "Fy", "Fz")])
+        op = orc.make_params(w.params, w.dx, nH_mean)
+        rel = (src_cell - torch.tensor(org)) % n                         # sources inside the sub-cube
+        inside = (rel < size).all(dim=1)
+        pos = ((rel[inside].double() + 0.5) / size).numpy()
+        rate = w.src_rate[inside].numpy()
+        orc.step(st, op, w.dt, p_steps, pos, rate)
+        sl = slice(p_steps, p_steps + m)
+        inner_org = tuple(o + p_steps for o in org)
+        g = {k: wl.cut_subcube(out[k], inner_org, m).numpy() for k in out}
+        ref = type("S", (), {k: getattr(st, k)[sl, sl, sl] for k in ("N", "Fx", "Fy", "Fz", "x", "T")})
+        err = l1_errors(g, ref, op.c)
+        for k, e in err.items():
+            worst[k] = max(worst.get(k, 0.0), e)
+        assert max(err[k] for k in ("N", "F", "x", "T")) <= TOL_L1, (state_name, org, int(inside.sum()), err)
+        # cell by cell (8 fp32 steps; 1e-4 is the 1-step bar from an oracle-evolved state): at most 0.2 % of
+        # the cells beyond 1e-3 in x and T, 1 % in N.  Those few are (i) extreme-density source cells (n_H ~ 1 cm^-3, C_R ~ 1e4,
+        # 50-70 sub-cycles per step) where heating and cooling nearly cancel, so the 10 % rule's sub-step
+        # eps E/|H - Lambda| is ill-conditioned and the fp32 and fp64 sub-step sequences separate at the
+        # truncation level of the first-order sub-step (per cent), and (ii) leading-edge cells of a front,
+        # where the upwind difference N - G_d cancels (H4/H5).  The reference kernel (variant 0)
+        # shows the same errors in the same cells: they belong to the fp32 formulation, not to the tiling.
+        big = ref.N > 1e-20 * max(ref.N.max(), 1e-300)
+        rel = {"x": np.abs(g["x"] - ref.x) / ref.x, "T": np.abs(g["T"] - ref.T) / ref.T}
+        if big.any():
+            rel["N"] = np.abs(g["N"][big] - ref.N[big]) / ref.N[big]
+        for k, e in rel.items():
+            assert np.mean(e > 1e-3) <= (1e-2 if k == "N" else 2e-3) and e.max() <= 0.5, (state_name, org, k, e.max(), float(np.mean(e > 1e-3)))
+    return worst
+
+
+@pytest.mark.skipif(not torch.cuda.is_available() or torch.cuda.get_device_properties(0).total_memory < 150e9,
+                    reason="needs the 1024^3 working set (about 110 GB of HBM)")
+def test_config5_full_size_subcubes_against_oracle(orc):
+    n, m, p_steps = 1024, 24, 8
+    w = wl.make_config(5, device="cuda")
+    nH_mean = float(w.nH.double().mean())
+    # sub-cubes: around the two brightest sources, across the periodic corner, across CTA / tile seams, a void
+    cells = (torch.floor(w.src_pos.double() * n).long() % n)
+    top = torch.argsort(w.src_rate, descending=True)[:2]
+    half = (m + 2 * p_steps) // 2
+    origins = [tuple(int(v) for v in ((cells[s] - half) % n)) for s in top]
+    origins += [(n - 20, n - 20, n - 20), (128 - 20, 4 * 37 - 20, 64 - 20)]
+    flat = int(torch.argmin(w.nH.reshape(-1)[: n * n * 64]))
+    origins.append(tuple(int(v) for v in ((torch.tensor([flat % n, (flat // n) % n, flat // (n * n)]) - half) % n)))
+    dark = _subcube_check(orc, w, "dark", origins, m, p_steps, nH_mean)
+    ww = wl.synthetic_warm_state(w)
+    del w
+    torch.cuda.empty_cache()
+    warm = _subcube_check(orc, ww, "warm", origins, m, p_steps, nH_mean)
+    print("worst relative L1 on sub-cubes: dark", dark, "warm", warm)
