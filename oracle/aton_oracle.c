@@ -46,6 +46,8 @@ typedef struct {
     double redshift;     /* <0: no Compton cooling */
     double eps_sub;      /* sub-cycle energy tolerance (Anninos 10% rule), reading S5 */
     double nH_mean;      /* <n_H>_V used by the linear clumping law, reading S8 */
+    double clump_i_a, clump_i_b; /* photo-ionisation clumping C_I = max(1, a nH^b) of Eq.15 (L247-249, L269:
+                                    "C_I ~ n_H^0.2"); a <= 0: C_I = 1 (reading S8b) */
     int recomb_case;     /* 1: case B, on-the-spot; 0: case A + recombination radiation (S6) */
     int cooling;         /* 0: T frozen; 1: heating + cooling */
     int coll_ion;        /* collisional ionisation on/off */
@@ -209,6 +211,14 @@ double orc_clumping(double nH, const orc_params *p) {
     return C > 1.0 ? C : 1.0;
 }
 
+/* photon-atom cross clumping factor C_I of Eq.15 (L247-249): multiplies the photo-ionisation rate and,
+ * so that every absorbed photon still ionises one atom, the absorption of N and F (reading S8b). */
+double orc_clumping_i(double nH, const orc_params *p) {
+    double C = 1.0;
+    if (p->clump_i_a > 0.0) C = p->clump_i_a * pow(nH, p->clump_i_b);
+    return C > 1.0 ? C : 1.0;
+}
+
 /* cooling function Lambda [erg cm^-3 s^-1] and its d/dlnT, at ionised fraction x, temperature T */
 static void cooling_fn(double x, double T, double nH, double CR, const orc_rates_t *r,
                        const orc_params *p, double *Lam, double *Lam_T) {
@@ -231,8 +241,8 @@ static void cooling_fn(double x, double T, double nH, double CR, const orc_rates
  * O4 one chemistry sub-step of length dts (steps 4-5 of the algorithm in DESIGN.md / SURVEY O4):
  * backward-Euler, photon-conserving coupled update of (N, x) with lagged n_e and T, then the
  * linearly-implicit energy update.  In/out: N, F[3], x, T.  Returns absorbed photons per cm^3.
- *   dN/dt = -c sigma_n n_H (1-x) N + S_rec                         (kappa terms of Eq.3-4)
- *   dx/dt = (1-x)(c sigma_n N + beta n_e) - alpha C_R n_e x        (Eq.14-15, reading G2)
+ *   dN/dt = -c sigma_n C_I n_H (1-x) N + S_rec                     (kappa terms of Eq.3-4)
+ *   dx/dt = (1-x)(c sigma_n C_I N + beta n_e) - alpha C_R n_e x    (Eq.14-15, readings G2, S8b)
  * ------------------------------------------------------------------------------------------- */
 double orc_chem_substep(double *N, double F[3], double *x_io, double *T_io, double nH, double dts,
                         const orc_params *p) {
@@ -246,7 +256,7 @@ double orc_chem_substep(double *N, double F[3], double *x_io, double *T_io, doub
     double S_rec = p->recomb_case == 1 ? 0.0 : (r.alpha_A - r.alpha_B) * CR * ne * x * nH;
     double E = 1.5 * K_BOLTZ * nH * (1.0 + x) * T;
 
-    double A = p->c * p->sigma_n * nH * dts;
+    double A = p->c * p->sigma_n * orc_clumping_i(nH, p) * nH * dts;
     double b = dts * beta * ne;
     double rr = dts * alpha * CR * ne;
     double L = 1.0 + b + rr;
@@ -285,7 +295,7 @@ static double edot_est(double N, double x, double T, double nH, const orc_params
     orc_rates(T, &r);
     double CR = orc_clumping(nH, p);
     double e_erg = p->e_photon_eV * EV_ERG, e0 = E0_EV * EV_ERG;
-    double H = nH * (1.0 - x) * p->c * N * (e_erg * p->sigma_e - e0 * p->sigma_n);
+    double H = nH * (1.0 - x) * p->c * orc_clumping_i(nH, p) * N * (e_erg * p->sigma_e - e0 * p->sigma_n);
     double Lam, Lam_T;
     cooling_fn(x, T, nH, CR, &r, p, &Lam, &Lam_T);
     return H - Lam;

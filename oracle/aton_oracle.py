@@ -32,7 +32,8 @@ class Params(C.Structure):
     _fields_ = [("c", C.c_double), ("dx", C.c_double), ("sigma_n", C.c_double),
                 ("sigma_e", C.c_double), ("e_photon_eV", C.c_double), ("clump_a", C.c_double),
                 ("clump_b", C.c_double), ("redshift", C.c_double), ("eps_sub", C.c_double),
-                ("nH_mean", C.c_double), ("recomb_case", C.c_int), ("cooling", C.c_int),
+                ("nH_mean", C.c_double), ("clump_i_a", C.c_double), ("clump_i_b", C.c_double),
+                ("recomb_case", C.c_int), ("cooling", C.c_int),
                 ("coll_ion", C.c_int), ("clump_model", C.c_int), ("max_sub", C.c_int)]
 
 
@@ -58,6 +59,8 @@ def lib():
         L.orc_rates.argtypes = [C.c_double, C.POINTER(Rates)]
         L.orc_clumping.restype = C.c_double
         L.orc_clumping.argtypes = [C.c_double, C.POINTER(Params)]
+        L.orc_clumping_i.restype = C.c_double
+        L.orc_clumping_i.argtypes = [C.c_double, C.POINTER(Params)]
         L.orc_chem_substep.restype = C.c_double
         L.orc_chem_substep.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, C.POINTER(Params)]
         L.orc_chem_cell.restype = C.c_int
@@ -87,6 +90,7 @@ def make_params(params: Dict[str, float], dx: float, nH_mean: float = 1.0) -> Pa
                   e_photon_eV=params["e_photon_eV"], clump_a=params.get("clump_a", 1.0),
                   clump_b=params.get("clump_b", 2.0), redshift=params.get("redshift", -1.0),
                   eps_sub=params.get("eps_sub", 0.1) or 0.1, nH_mean=nH_mean,
+                  clump_i_a=params.get("clump_i_a", 0.0), clump_i_b=params.get("clump_i_b", 0.0),
                   recomb_case=int(params.get("recomb_case", 1)), cooling=int(params.get("cooling", 1)),
                   coll_ion=int(params.get("coll_ion", 1)), clump_model=int(params.get("clump_model", 0)),
                   max_sub=int(params.get("max_sub", 1 << 14) or (1 << 14)))
@@ -136,6 +140,10 @@ def rates(T: float) -> Dict[str, float]:
 
 def clumping(nH: float, p: Params) -> float:
     return float(lib().orc_clumping(float(nH), C.byref(p)))
+
+
+def clumping_i(nH: float, p: Params) -> float:
+    return float(lib().orc_clumping_i(float(nH), C.byref(p)))
 
 
 def chem_substep(N: float, F, x: float, T: float, nH: float, dts: float, p: Params):

@@ -27,6 +27,9 @@
 
 namespace aton {
 
+#ifndef ATON_V4_WARPS
+#define ATON_V4_WARPS 4
+#endif
 struct V4Cfg {
     static constexpr int WX = 32, WY = 4;                // cells per warp tile
     static constexpr int RS = 40;                        // raw row: quads at col 4 + 4q, x halos at 3 and 36
@@ -35,7 +38,7 @@ struct V4Cfg {
     static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
     static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][32]
     static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN;
-    static constexpr int WARPS = 4, THREADS = 32 * WARPS;
+    static constexpr int WARPS = ATON_V4_WARPS, THREADS = 32 * WARPS;
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
 };
 

@@ -81,6 +81,10 @@ def test_clumping_laws(orc):
     assert orc.clumping(0.5, p) == 1.0                                         # 1+2 delta < 1 clamps
     p = _params(orc, clump_model=2, clump_a=30.0, clump_b=0.7)                 # K nH^0.7 (L259)
     assert orc.clumping(0.1, p) == pytest.approx(30.0 * 0.1 ** 0.7)
+    assert orc.clumping_i(0.1, p) == 1.0                                       # C_I off by default (L269-271)
+    p = _params(orc, clump_i_a=4.0, clump_i_b=0.2)                             # K nH^0.2 (L269)
+    assert orc.clumping_i(0.1, p) == pytest.approx(4.0 * 0.1 ** 0.2)
+    assert orc.clumping_i(1e-9, p) == 1.0                                      # never below 1
 
 
 # ------------------------------------------------------------------ the backward-Euler sub-step
@@ -91,45 +95,49 @@ def _draw(rng):
                 T=10 ** rng.uniform(1.5, 6), nH=nH, dts=10 ** rng.uniform(8, 13))
 
 
-def _implicit_residual(yp, d, p, r, CR, case_b, coll):
-    """x' - x - dts[ y'(c sigma N' + beta n_e) - alpha C_R n_e x' ], N' from backward Euler."""
+def _implicit_residual(yp, d, p, r, CR, case_b, coll, CI=1.0):
+    """x' - x - dts[ y'(c sigma C_I N' + beta n_e) - alpha C_R n_e x' ], N' from backward Euler."""
     x, y = d["x"], 1 - d["x"]
     ne = x * d["nH"]
     alpha = r["alpha_B"] if case_b else r["alpha_A"]
     beta = r["beta"] if coll else 0.0
     S = 0.0 if case_b else (r["alpha_A"] - r["alpha_B"]) * CR * ne * x * d["nH"]
-    A = p.c * p.sigma_n * d["nH"] * d["dts"]
+    A = p.c * p.sigma_n * CI * d["nH"] * d["dts"]
     Np = (d["N"] + d["dts"] * S) / (1 + A * yp)
     xp = 1 - yp
-    return (xp - x) - d["dts"] * (yp * (p.c * p.sigma_n * Np + beta * ne) - alpha * CR * ne * xp), Np
+    return (xp - x) - d["dts"] * (yp * (p.c * p.sigma_n * CI * Np + beta * ne) - alpha * CR * ne * xp), Np
 
 
-@pytest.mark.parametrize("case_b,coll,clump", [(1, 1, 0), (0, 1, 1), (1, 0, 0), (0, 0, 1)])
-def test_substep_solves_the_implicit_system_and_conserves_photons(orc, case_b, coll, clump):
+@pytest.mark.parametrize("case_b,coll,clump,ci", [(1, 1, 0, 0), (0, 1, 1, 0), (1, 0, 0, 0), (0, 0, 1, 0),
+                                                  (0, 1, 1, 1), (1, 1, 0, 1)])
+def test_substep_solves_the_implicit_system_and_conserves_photons(orc, case_b, coll, clump, ci):
     """P5: the closed-form quadratic root equals the unique root in (0,1] of the backward-Euler
     system found by bisection; and N' + nH x' = N + nH x + dts S_rec + nH (b y' - r x') exactly."""
-    rng = np.random.default_rng(10 + case_b * 2 + coll)
-    p = _params(orc, recomb_case=case_b, coll_ion=coll, clump_model=clump, cooling=0, nH_mean=1e-3)
+    rng = np.random.default_rng(10 + case_b * 2 + coll + 7 * ci)
+    p = _params(orc, recomb_case=case_b, coll_ion=coll, clump_model=clump, cooling=0, nH_mean=1e-3,
+                clump_i_a=(40.0 if ci else 0.0), clump_i_b=0.2)
     for _ in range(400):
         d = _draw(rng)
         r = orc.rates(d["T"])
         CR = orc.clumping(d["nH"], p)
+        CI = orc.clumping_i(d["nH"], p)
+        assert CI == (max(1.0, 40.0 * d["nH"] ** 0.2) if ci else 1.0)
         F0 = np.array([0.3, -0.2, 0.1]) * C * d["N"]
         Nn, Fn, xn, Tn, absorbed = orc.chem_substep(d["N"], F0, d["x"], d["T"], d["nH"], d["dts"], p)
         assert 0.0 <= xn <= 1.0 and Nn >= 0.0 and Tn == d["T"]
         # brute force: bisection on y' in [0, 1]
         lo, hi = 0.0, 1.0
-        flo = _implicit_residual(lo, d, p, r, CR, case_b, coll)[0]
-        fhi = _implicit_residual(hi, d, p, r, CR, case_b, coll)[0]
+        flo = _implicit_residual(lo, d, p, r, CR, case_b, coll, CI)[0]
+        fhi = _implicit_residual(hi, d, p, r, CR, case_b, coll, CI)[0]
         assert flo >= 0 >= fhi
         for _ in range(200):
             mid = 0.5 * (lo + hi)
-            if _implicit_residual(mid, d, p, r, CR, case_b, coll)[0] > 0:
+            if _implicit_residual(mid, d, p, r, CR, case_b, coll, CI)[0] > 0:
                 lo = mid
             else:
                 hi = mid
         yb = 0.5 * (lo + hi)
-        Nb = _implicit_residual(yb, d, p, r, CR, case_b, coll)[1]
+        Nb = _implicit_residual(yb, d, p, r, CR, case_b, coll, CI)[1]
         assert (1 - xn) == pytest.approx(yb, rel=1e-7, abs=1e-13)
         assert Nn == pytest.approx(Nb, rel=1e-6, abs=1e-300)
         # photon budget identity
@@ -140,12 +148,12 @@ def test_substep_solves_the_implicit_system_and_conserves_photons(orc, case_b, c
         S = 0.0 if case_b else (r["alpha_A"] - r["alpha_B"]) * CR * ne * d["x"] * d["nH"]
         lhs = Nn + d["nH"] * xn
         rhs = d["N"] + d["nH"] * d["x"] + d["dts"] * S + d["nH"] * (b * (1 - xn) - rr * xn)
-        assert lhs == pytest.approx(rhs, rel=1e-10)
+        assert lhs == pytest.approx(rhs, rel=1e-10 * max(1.0, CI) ** 2)      # root conditioning grows with A
         assert absorbed == pytest.approx(d["N"] + d["dts"] * S - Nn, rel=1e-6, abs=1e-14 * d["nH"])
         # flux attenuated by 1/(1 + A y'): same factor as N when S_rec = 0 (f unchanged)
         if d["N"] > 0:
             assert np.allclose(Fn / F0, Nn / (d["N"] + d["dts"] * S), rtol=1e-12)
-        A = p.c * p.sigma_n * d["nH"] * d["dts"]
+        A = p.c * p.sigma_n * CI * d["nH"] * d["dts"]
         assert np.allclose(Fn, F0 / (1 + A * (1 - xn)), rtol=1e-5)
 
 
@@ -156,6 +164,31 @@ def test_absorbed_photons_equal_ionisations_without_recombination(orc):
     Nn, _, xn, _, ab = orc.chem_substep(N, [0, 0, 0], x, 1e9, nH, dts, p)
     assert (xn - x) * nH == pytest.approx(N - Nn, rel=1e-6)
     assert ab == pytest.approx(N - Nn, rel=1e-12)
+
+
+def test_photoionisation_equilibrium_with_ionisation_clumping(orc):
+    """Eq.15 (L247-249) with C_I: the steady state satisfies alpha C_R nH x^2 = (1-x)(c sigma_n C_I N + beta nH x)
+    whatever dts, i.e. the equilibrium of a gas seeing C_I times the photon density."""
+    nH, T, N0 = 3e-4, 2.0e4, 1e-9
+    p = _params(orc, cooling=0, coll_ion=1, clump_model=2, clump_a=30.0, clump_b=0.7, clump_i_a=20.0, clump_i_b=0.2)
+    r = orc.rates(T)
+    CR, CI = orc.clumping(nH, p), orc.clumping_i(nH, p)
+    assert CI == pytest.approx(20.0 * nH ** 0.2) and CI > 1.0
+    xs = []
+    for dts in (1e9, 1e11, 3e12):
+        x = 0.3
+        for _ in range(20000):
+            Nn, _, x, _, _ = orc.chem_substep(N0, [0, 0, 0], x, T, nH, dts, p)
+        G = p.c * p.sigma_n * CI * Nn
+        assert r["alpha_B"] * CR * nH * x * x == pytest.approx((1 - x) * (G + r["beta"] * nH * x), rel=1e-9)
+        xs.append(x)
+    # the same gas without C_I but with N0 -> C_I N0 and sigma -> sigma (absorption C_I times weaker per photon):
+    # identical rate equation for x at fixed N', so x differs only through N' (checked above via G)
+    p1 = _params(orc, cooling=0, coll_ion=1, clump_model=2, clump_a=30.0, clump_b=0.7)
+    x = 0.3
+    for _ in range(20000):
+        Nn1, _, x, _, _ = orc.chem_substep(N0, [0, 0, 0], x, T, nH, 1e9, p1)
+    assert x < xs[0]                       # clumping of the photons ionises more
 
 
 @pytest.mark.parametrize("clump", [0, 1])
