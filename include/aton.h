@@ -60,6 +60,9 @@ typedef struct {
     double redshift;     /* >= 0: Compton cooling off the CMB at this z; < 0: off */
     double eps_sub;      /* sub-cycle tolerance on the thermal energy change; 0 => 0.1 */
     int max_sub;         /* sub-cycle cap per cell and step; 0 => 16384 */
+    double clump_i_a, clump_i_b; /* photon-atom cross clumping C_I of Eq.15 ("C_I ~ n_H^0.2"):
+                            C_I = max(1, a * n_H^b) multiplies the photo-ionisation rate and the absorption;
+                            a <= 0 => C_I = 1 (the variant the paper also ran, L269-271) */
 } aton_params_t;
 
 /* Global diagnostics (PAPER.md:L149 volume-weighted x, L303-305 mass-weighted, Eq.15 Gamma = c sigma_n N). */

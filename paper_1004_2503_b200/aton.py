@@ -35,7 +35,7 @@ class Params(C.Structure):
                 ("e_photon_eV", C.c_double), ("recomb_case", C.c_int), ("cooling", C.c_int),
                 ("coll_ion", C.c_int), ("clump_model", C.c_int), ("clump_a", C.c_double),
                 ("clump_b", C.c_double), ("redshift", C.c_double), ("eps_sub", C.c_double),
-                ("max_sub", C.c_int)]
+                ("max_sub", C.c_int), ("clump_i_a", C.c_double), ("clump_i_b", C.c_double)]
 
 
 class Diag(C.Structure):

@@ -112,6 +112,8 @@ StepConst make_step_const(const aton_ctx *ctx, double dt) {
         s.clump_k0 = (float)p.clump_a;
         s.clump_k1 = (float)p.clump_b;
     }
+    s.ci_k0 = p.clump_i_a > 0.0 ? (float)p.clump_i_a : 0.0f;
+    s.ci_k1 = (float)p.clump_i_b;
     s.inj_scale = 0.0f;
     return s;
 }

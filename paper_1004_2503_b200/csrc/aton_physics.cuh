@@ -33,6 +33,7 @@ struct StepConst {        // per aton_step call, host-computed in fp64, passed b
     int max_sub;
     int clump_model;
     float clump_k0, clump_k1;  // model 1: C = max(1, k0 + k1*nH); model 2: C = max(1, k0 * nH^k1)
+    float ci_k0, ci_k1;   // C_I = max(1, k0 * nH^k1) on photo-ionisation and absorption; k0 <= 0: off (C_I = 1)
     float inj_scale;      // dt / dx^3 folded into the per-source density rate
 };
 
@@ -142,6 +143,11 @@ __device__ __forceinline__ float clumping(float nH, const StepConst &c) {
     return fmaxf(C, 1.0f);
 }
 
+// photon-atom cross clumping factor C_I of Eq.15
+__device__ __forceinline__ float clumping_i(float nH, const StepConst &c) {
+    return fmaxf(c.ci_k0 * f_ex2(c.ci_k1 * f_lg2(nH)), 1.0f);
+}
+
 // ---------------------------------------------------------------- O4 chemistry / cooling
 // In/out: N, G (=F/c), x, T after transport + injection; nH fixed.  Returns the sub-cycle count.
 template <int FLAGS>
@@ -150,7 +156,10 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
     constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL;
     const float CR = clumping(nH, c);
     const float inv_nH = f_rcp(nH);
-    const float cs_nH = c.cs * nH;
+    const bool ci_on = c.ci_k0 > 0.0f;
+    const float CI = ci_on ? clumping_i(nH, c) : 1.0f;
+    const float cs_nH = ci_on ? c.cs * nH * CI : c.cs * nH;
+    const float heat_rate = ci_on ? c.heat_rate_K * CI : c.heat_rate_K;
     float t_left = c.dt;
     int nsub = 0;
     float att_tot = 1.0f;
@@ -164,7 +173,7 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
         if (COOL) {
             // estimated net heating rate / (1.5 kB nH)  [K/s]
             float lamK = nH * (x * x * fmaf(CR, r.zrec, r.zff) + x * y * r.zxy) + c.compton0 * x * (T - c.t_cmb);
-            float ed = fabsf(y * N * c.heat_rate_K - lamK);
+            float ed = fabsf(y * N * heat_rate - lamK);
             if (ed * t_left > c.eps_sub * theta) dts = c.eps_sub * theta / ed;
         }
         // backward-Euler coupled (N, x) update, solved for delta = x' - x

@@ -118,6 +118,13 @@ __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2
     Rates2 r;
     rates2<FLAGS>(T, warm, c, r);
     const f2 CR = clumping2(nH, c);
+    const bool ci_on = c.ci_k0 > 0.0f;                                    // uniform: C_I of Eq.15, off by default
+    f2 nHs = nH, Ns = N;                                                  // C_I nH (absorbers seen by the photons), C_I N
+    if (ci_on) {
+        const f2 CI = max2(ex22(lg22(nH) * c.ci_k1) * c.ci_k0, 1.0f);
+        nHs = nH * CI;
+        Ns = N * CI;
+    }
     const f2 y = 1.0f - x;
     const f2 ne = x * nH;
     const f2 theta = fma2(x, T, T);                                      // (1 + x) T
@@ -126,13 +133,13 @@ __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2
     if (COOL) {
         // estimated net heating rate / (1.5 kB nH) [K/s]: the Anninos 10 % rule decides on sub-cycling
         const f2 lamK = fma2(nH, (x * x) * crz + (x * y) * r.zxy, (x * c.compton0) * (T - c.t_cmb));
-        const f2 ed = abs2(fma2(y * N, c.heat_rate_K, splat(0.0f) - lamK));
+        const f2 ed = abs2(fma2(y * Ns, c.heat_rate_K, splat(0.0f) - lamK));
         const f2 lhs = ed * c.dt, rhs = theta * c.eps_sub;
         defer |= (lo(lhs) > lo(rhs) ? 1u : 0u) | (hi(lhs) > hi(rhs) ? 2u : 0u);
     }
     // backward-Euler coupled (N, x) update, solved for delta = x' - x
     const float dt = c.dt;
-    const f2 A = (nH * c.cs) * dt;
+    const f2 A = (nHs * c.cs) * dt;
     const f2 dne = ne * dt;
     const f2 b = dne * r.beta;
     const f2 ane = (r.alpha * CR) * dne;                                  // rr = dt alpha C_R n_e

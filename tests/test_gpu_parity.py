@@ -92,7 +92,9 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
     """The other physics-switch combinations (template instantiations) against the oracle."""
     for kw in (dict(cooling=0, coll_ion=0), dict(cooling=0, coll_ion=1, recomb_case=0),
                dict(cooling=1, coll_ion=0, recomb_case=0, clump_model=2, clump_a=3.0, clump_b=0.2),
-               dict(cooling=1, coll_ion=0, redshift=9.0)):
+               dict(cooling=1, coll_ion=0, redshift=9.0),
+               # paper-form clumping (Eq.15, L247-271): C_R = K nH^0.7 and C_I = K' nH^0.2
+               dict(cooling=1, coll_ion=1, recomb_case=0, clump_model=2, clump_a=300.0, clump_b=0.7, clump_i_a=8.0, clump_i_b=0.2)):
         w = twin(3, 32, 60)
         w.params.update(kw)
         ww = _warm(orc, w, 40)
@@ -253,7 +255,7 @@ def test_empty_sources_and_vacuum_conservation():
 # for it (they run the variant-2 kernel under the default variant), so it gets non-cubic grids whose
 # x extent spans one or two 128-cell tiles, several y tiles and a ragged z chunk.
 # ------------------------------------------------------------------------------------------------
-def _slab_case(nx, ny, nz, flags7, seed):
+def _slab_case(nx, ny, nz, flags7, seed, paper_clumping=False):
     """Random log-normal-ish density on an (nz, ny, nx) grid, sources on tile corners / edges, physics of
     config 4 (flags7: case A + recombination radiation + clumping) or config 2 (case B)."""
     rng = np.random.default_rng(seed)
@@ -264,6 +266,8 @@ def _slab_case(nx, ny, nz, flags7, seed):
     p.update(redshift=8.0)
     if flags7:
         p.update(recomb_case=0, clump_model=1, clump_a=1.0, clump_b=2.0)
+    if paper_clumping:      # Eq.15 with the fitted trends C_R ~ nH^0.7, C_I ~ nH^0.2 (L259, L269)
+        p.update(clump_model=2, clump_a=300.0, clump_b=0.7, clump_i_a=8.0, clump_i_b=0.2)
     dx = 3.0e21
     cells = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (127 % nx, 7 % ny, 1 % nz), (128 % nx, 8 % ny, 2 % nz), (nx // 2, ny // 2, nz // 2),
              (3, ny - 1, 0), (nx - 4, 0, nz - 1)]
@@ -290,12 +294,12 @@ def _run_slab(variant, tile, nH, x, T, p, dx, pos, rate, n_steps, rad=None):
 @pytest.mark.parametrize("variant,shape,flags7",
                          [(3, (128, 16, 11), True), (3, (256, 24, 9), False), (3, (128, 8, 3), True),
                           (4, (128, 16, 11), True), (4, (256, 24, 9), False), (4, (32, 8, 5), True),
-                          (4, (160, 12, 1), True), (4, (64, 4, 70), False)],
+                          (4, (160, 12, 1), True), (4, (64, 4, 70), False), (4, (96, 8, 7), "paper")],
                          ids=["v3_128x16x11_A", "v3_256x24x9_B", "v3_128x8x3_A", "v4_128x16x11_A", "v4_256x24x9_B",
-                              "v4_32x8x5_A", "v4_160x12x1_A", "v4_64x4x70_B"])
+                              "v4_32x8x5_A", "v4_160x12x1_A", "v4_64x4x70_B", "v4_96x8x7_paper_clumping"])
 def test_full_tile_kernels_against_oracle(orc, variant, shape, flags7):
     nx, ny, nz = shape
-    nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, flags7, seed=nx + ny + nz)
+    nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, bool(flags7), seed=nx + ny + nz, paper_clumping=flags7 == "paper")
     dt = wl.courant_dt(dx)
     op = orc.make_params(p, dx, float(nH.astype(np.float64).mean()))
     zero = np.zeros_like(nH)
