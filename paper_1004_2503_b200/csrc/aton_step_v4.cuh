@@ -42,6 +42,27 @@ struct V4Cfg {
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
 };
 
+#ifndef ATON_V4_X
+#define ATON_V4_X 7      // codegen choices (measured: profiles/r01_d_step_v4.md); bits: 1 edge selects by slct; 2 predicated y stores; 4 predicated staging
+#endif
+// d = (c >= 0) ? a : b in one instruction
+__device__ __forceinline__ float slct(float a, float b, int c) {
+    float d;
+    asm("slct.f32.s32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ void sts128_if(float *p, float a, float b, float c, float d, int pred) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %5, 0;\n@p st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n}"
+                 ::"r"(smem_u32(p)), "f"(a), "f"(b), "f"(c), "f"(d), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void cp_async16_if(void *smem, const void *gmem, int pred) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %2, 0;\n@p cp.async.cg.shared.global [%0], [%1], 16;\n}"
+                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int pred) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %2, 0;\n@p cp.async.ca.shared.global [%0], [%1], 4;\n}"
+                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(pred) : "memory");
+}
 #ifndef ATON_V4_MINB
 #define ATON_V4_MINB 4
 #endif
@@ -83,6 +104,12 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
 #pragma unroll
         for (int v = 0; v < 4; v++) cp_async16(dst + v * C::RAW_FIELD + my, src[v] + base + rowoff);
         if (inpl) {
+#if ATON_V4_X & 4
+#pragma unroll
+            for (int v = 0; v < 4; v++) cp_async16_if(dst + v * C::RAW_FIELD + myh, src[v] + base + hoff, hbot || htop);
+#pragma unroll
+            for (int v = 0; v < 4; v++) cp_async4_if(dst + v * C::RAW_FIELD + mxh, src[v] + base + xoff, edge_l || edge_r);
+#else
             if (hbot || htop) {
 #pragma unroll
                 for (int v = 0; v < 4; v++) cp_async16(dst + v * C::RAW_FIELD + myh, src[v] + base + hoff);
@@ -91,6 +118,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
 #pragma unroll
                 for (int v = 0; v < 4; v++) cp_async4(dst + v * C::RAW_FIELD + mxh, src[v] + base + xoff);
             }
+#endif
         }
         cp_async_commit();
         kst = kst + 1 == g.nz ? 0 : kst + 1;
@@ -151,12 +179,17 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
                 for (int v = 0; v < 4; v++) {
                     const f2 p0 = u.v[0][v] + F[0][v], p1 = u.v[1][v] + F[1][v];
                     const f2 m0 = u.v[0][v] - F[0][v], m1 = u.v[1][v] - F[1][v];
+#if ATON_V4_X & 2
+                    sts128_if(wyp + v * C::W_COMP + (r + 1) * 32 + 4 * q, lo(p0), hi(p0), lo(p1), hi(p1), !htop);
+                    sts128_if(wym + v * C::W_COMP + (r - 1) * 32 + 4 * q, lo(m0), hi(m0), lo(m1), hi(m1), !hbot);
+#else
                     if (!htop)
                         *reinterpret_cast<float4 *>(wyp + v * C::W_COMP + (r + 1) * 32 + 4 * q) =
                             make_float4(lo(p0), hi(p0), lo(p1), hi(p1));
                     if (!hbot)
                         *reinterpret_cast<float4 *>(wym + v * C::W_COMP + (r - 1) * 32 + 4 * q) =
                             make_float4(lo(m0), hi(m0), lo(m1), hi(m1));
+#endif
                 }
             }
             // ---- the tile's y halo rows (lanes of rows 0 and 3; the others compute and store nothing new)
@@ -177,12 +210,18 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
                     for (int v = 0; v < 4; v++) w[p][v] = fma2(F[v], sg, e[v]);
                 }
                 float *wdst = hbot ? wyp + 4 * q : wym + (C::WY - 1) * 32 + 4 * q;
+#if ATON_V4_X & 2
+#pragma unroll
+                for (int v = 0; v < 4; v++)
+                    sts128_if(wdst + v * C::W_COMP, lo(w[0][v]), hi(w[0][v]), lo(w[1][v]), hi(w[1][v]), hbot || htop);
+#else
                 if (hbot || htop) {
 #pragma unroll
                     for (int v = 0; v < 4; v++)
                         *reinterpret_cast<float4 *>(wdst + v * C::W_COMP) =
                             make_float4(lo(w[0][v]), hi(w[0][v]), lo(w[1][v]), hi(w[1][v]));
                 }
+#endif
             }
             __syncwarp();                                // y terms of the plane are visible to the warp
         }
@@ -222,8 +261,13 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
             for (int v = 0; v < 4; v++) {
                 float left = __shfl_up_sync(0xffffffffu, hi(Wp[1][v]), 1);
                 float right = __shfl_down_sync(0xffffffffu, lo(Wm[0][v]), 1);
+#if ATON_V4_X & 1
+                left = slct(left, lo(eWp[v]), q - 1);         // q == 0: the halo cell
+                right = slct(right, lo(eWm[v]), 6 - q);       // q == 7: the halo cell
+#else
                 left = edge_l ? lo(eWp[v]) : left;
                 right = edge_r ? lo(eWm[v]) : right;
+#endif
                 const f2 sx0 = pk(left + hi(Wm[0][v]), lo(Wp[0][v]) + lo(Wm[1][v]));
                 const f2 sx1 = pk(hi(Wp[0][v]) + hi(Wm[1][v]), lo(Wp[1][v]) + right);
                 t.v[0][v] = fma2(sx0, c.h, t.v[0][v]);
