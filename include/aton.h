@@ -138,6 +138,36 @@ int aton_set_timing(aton_t *ctx, int on);
 /* Sum [ms] and number of the bracketed launches since aton_set_timing(ctx, 1).  Synchronises. */
 int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches);
 
+/* ---- slab decomposition along z (the paper's multi-GPU mode, PAPER.md:L471-484,
+ * re-cut as z slabs whose one-plane halo of (N, F) is one contiguous block per field) ----
+ *
+ * aton_init_slab creates a context that advances planes [z_begin, z_begin + nz_local) of the GLOBAL grid
+ * `global_grid` (needs nx % 32 == 0, ny % 4 == 0: kernel variant 4).  It holds nz_local + 2 planes per array: its
+ * own planes between a ghost plane below and one above.  aton_set_fields / aton_get_fields then take arrays of
+ * nz_local planes; aton_set_sources takes positions in the GLOBAL box and keeps the sources of the slab;
+ * aton_reduce reports the slab's own means.  Before EVERY aton_step(ctx, dt, 1) the caller exchanges halos:
+ *   aton_halo_pack(ctx, send_lo, send_hi)      own first / last plane of N, Gx, Gy, Gz -> two device buffers
+ *   (send_hi goes to the slab above as its recv_lo, send_lo to the slab below as its recv_hi; periodic in z;
+ *    how the buffers travel -- NCCL send/recv, peer copies -- is the caller's business)
+ *   aton_halo_unpack(ctx, recv_lo, recv_hi)    two device buffers -> ghost plane below / above
+ * Each buffer is [4][ny][nx] float32 on the device (fields N, Gx, Gy, Gz with G = F/c as carried internally).
+ * Both calls are asynchronous on the context's stream.  A slab run is bit-identical to the undivided run. */
+int aton_init_slab(aton_t **out, const aton_grid_t *global_grid, const aton_box_t *box,
+                   const aton_params_t *params, void *cuda_stream, int z_begin, int nz_local);
+int aton_halo_pack(aton_t *ctx, float *send_lo, float *send_hi);
+int aton_halo_unpack(aton_t *ctx, const float *recv_lo, const float *recv_hi);
+
+/* <n_H> of the linear clumping law (clump_model 1): aton_set_fields computes it over the context's own cells;
+ * a slab must be given the GLOBAL mean (all-reduced by the caller) before aton_set_fields or aton_step. */
+int aton_set_mean_density(aton_t *ctx, double nH_mean);
+
+/* Raw sums of the context's own cells, to be combined across slabs (sum entries 0-10, max 11-12, min 13):
+ * [0] cells [1] sum x [2] sum n_H x [3] sum n_H [4] sum N [5] sum n_H N [6] sum T [7] cells with x >= 0.5
+ * [8] non-finite cells [9] sub-cycles [10] cells redone by the fix-up [11] max f [12] max sub-cycles [13] min N.
+ * n must be ATON_NSUMS.  Synchronises. */
+#define ATON_NSUMS 14
+int aton_reduce_sums(aton_t *ctx, double *sums, int n);
+
 void aton_free(aton_t *ctx);
 
 /* Message of the last failing call on ctx (ctx-owned), or of the last failing aton_init if ctx is

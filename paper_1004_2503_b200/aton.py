@@ -19,7 +19,9 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt", "aton_step",
            "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_set_timing",
-           "aton_kernel_time", "aton_free", "aton_last_error")
+           "aton_kernel_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
+           "aton_reduce_sums", "aton_free", "aton_last_error")
+NSUMS = 14
 
 
 class Grid(C.Structure):
@@ -89,6 +91,16 @@ def load_library(path: Optional[str] = None):
     L.aton_set_timing.argtypes = [vp, C.c_int]
     L.aton_kernel_time.restype = C.c_int
     L.aton_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.aton_init_slab.restype = C.c_int
+    L.aton_init_slab.argtypes = [C.POINTER(vp), C.POINTER(Grid), C.POINTER(Box), C.POINTER(Params), vp, C.c_int, C.c_int]
+    L.aton_halo_pack.restype = C.c_int
+    L.aton_halo_pack.argtypes = [vp, fp, fp]
+    L.aton_halo_unpack.restype = C.c_int
+    L.aton_halo_unpack.argtypes = [vp, fp, fp]
+    L.aton_set_mean_density.restype = C.c_int
+    L.aton_set_mean_density.argtypes = [vp, C.c_double]
+    L.aton_reduce_sums.restype = C.c_int
+    L.aton_reduce_sums.argtypes = [vp, C.POINTER(C.c_double), C.c_int]
     L.aton_free.restype = None
     L.aton_free.argtypes = [vp]
     L.aton_last_error.restype = C.c_char_p
@@ -119,16 +131,22 @@ class Aton:
     """One simulation context (aton_t).  Methods mirror the C entry points one to one."""
 
     def __init__(self, nx: int, ny: int, nz: int, lx_cm: float, params: Dict[str, float],
-                 stream: Optional[torch.cuda.Stream] = None):
+                 stream: Optional[torch.cuda.Stream] = None, slab=None):
+        """`slab` = (z_begin, nz_local): aton_init_slab on planes [z_begin, z_begin + nz_local) of the global grid."""
         self._L = load_library()
         self._h = C.c_void_p()
-        self.shape = (nz, ny, nx)
-        self.ncell = nx * ny * nz
+        nz_own = nz if slab is None else int(slab[1])
+        self.shape = (nz_own, ny, nx)
+        self.ncell = nx * ny * nz_own
+        self.plane = nx * ny
         self._stream = stream
         sp = C.c_void_p(stream.cuda_stream if stream is not None
                         else (torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0))
         g, b, p = Grid(nx, ny, nz), Box(lx_cm), make_params(params)
-        rc = self._L.aton_init(C.byref(self._h), C.byref(g), C.byref(b), C.byref(p), sp)
+        if slab is None:
+            rc = self._L.aton_init(C.byref(self._h), C.byref(g), C.byref(b), C.byref(p), sp)
+        else:
+            rc = self._L.aton_init_slab(C.byref(self._h), C.byref(g), C.byref(b), C.byref(p), sp, int(slab[0]), int(slab[1]))
         if rc != OK:
             self._h = C.c_void_p()
             raise AtonError(rc, self._L.aton_last_error(None).decode())
@@ -189,6 +207,22 @@ class Aton:
 
     def set_kernel(self, variant: int, tile_y: int = 0, tile_z: int = 0):
         self._check(self._L.aton_set_kernel(self._h, variant, tile_y, tile_z))
+
+    def halo_pack(self, send_lo: torch.Tensor, send_hi: torch.Tensor):
+        self._check(self._L.aton_halo_pack(self._h, _ptr(send_lo, 4 * self.plane, torch.float32, True),
+                                           _ptr(send_hi, 4 * self.plane, torch.float32, True)))
+
+    def halo_unpack(self, recv_lo: torch.Tensor, recv_hi: torch.Tensor):
+        self._check(self._L.aton_halo_unpack(self._h, _ptr(recv_lo, 4 * self.plane, torch.float32, True),
+                                             _ptr(recv_hi, 4 * self.plane, torch.float32, True)))
+
+    def set_mean_density(self, nH_mean: float):
+        self._check(self._L.aton_set_mean_density(self._h, float(nH_mean)))
+
+    def reduce_sums(self):
+        buf = (C.c_double * NSUMS)()
+        self._check(self._L.aton_reduce_sums(self._h, buf, NSUMS))
+        return list(buf)
 
     def set_timing(self, on: bool):
         self._check(self._L.aton_set_timing(self._h, int(bool(on))))

@@ -34,7 +34,11 @@ char g_init_error[512] = "";
 
 struct aton_ctx {
     Grid g{};
-    size_t ncell = 0;
+    size_t ncell = 0;                      // cells this context advances (the slab's own planes)
+    size_t nalloc = 0, plane = 0, off = 0; // allocated cells per array (slab: + 2 ghost planes), nx*ny, first own cell
+    bool slab = false;                     // aton_init_slab: planes [z_begin, z_begin + nz_local) of a global grid
+    int z_begin = 0, nz_local = 0, nz_global = 0;
+    bool mean_set = false;                 // aton_set_mean_density overrides <n_H> of aton_set_fields
     double dx = 0, c = 0;
     aton_params_t p{};
     cudaStream_t stream = nullptr;
@@ -146,7 +150,7 @@ template <int FLAGS>
 cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
     if (ctx->variant == 0) {
         const int threads = 256;
-        const unsigned blocks = (unsigned)((ctx->ncell + threads - 1) / threads);
+        const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
         time_mark(ctx);
         step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc);
         time_mark(ctx);
@@ -161,11 +165,13 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
     // variant 4 needs nx % 32 == 0, ny % 4 == 0; variant 3 nx % 128 == 0, ny % TY == 0; other grids run the
     // variant-2 kernel.  Only variant 4 leaves the source injection to the fix-up kernel.
     const bool use4 = ctx->variant == 4 && v4_grid_ok(ctx->g);
+    if (ctx->slab && !use4) return cudaErrorNotSupported;    // checked with a message in aton_step
     const int ty3 = ctx->variant == 3 ? v3_pick_ty(ctx->g, ctx->tile_y) : 0;
     FieldsIO f2 = f;
     f2.fix_inject = use4 ? 1 : 0;
     time_mark(ctx);
-    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, ctx->tile_z, ctx->stream)
+    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
+                                                 ctx->slab ? ctx->nz_local + 1 : ctx->g.nz)
                     : ty3 ? launch_step_v3<FLAGS>(f2, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
                           : launch_step_fused<FLAGS>(f2, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0,
                                                      ctx->variant == 2 ? ctx->tile_z : 0, ctx->stream);
@@ -207,9 +213,11 @@ int run_reduce(aton_ctx *ctx, bool full, double *host_out) {
     const int nquad = (int)(ctx->ncell / 4);
     const int blocks = std::min((nquad + 255) / 256, REDUCE_BLOCKS);
     float **r = ctx->rad[ctx->cur];
+    const size_t o = ctx->off;             // the slab's own planes start one plane in
     reduce_pass1<<<blocks, 256, 0, ctx->stream>>>(
-        full ? (const float4 *)r[0] : nullptr, (const float4 *)r[1], (const float4 *)r[2], (const float4 *)r[3],
-        (const float4 *)ctx->x, (const float4 *)ctx->T, (const float4 *)ctx->nH, nquad, ctx->partials);
+        full ? (const float4 *)(r[0] + o) : nullptr, (const float4 *)(r[1] + o), (const float4 *)(r[2] + o),
+        (const float4 *)(r[3] + o), (const float4 *)(ctx->x + o), (const float4 *)(ctx->T + o),
+        (const float4 *)(ctx->nH + o), nquad, ctx->partials);
     CU(ctx, cudaGetLastError());
     double *out = ctx->partials + (size_t)REDUCE_BLOCKS * R_COUNT;
     reduce_pass2<<<1, 32, 0, ctx->stream>>>(ctx->partials, blocks, out);
@@ -224,15 +232,21 @@ int run_reduce(aton_ctx *ctx, bool full, double *host_out) {
 
 extern "C" {
 
-int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, const aton_params_t *params,
-              void *cuda_stream) {
+static int init_common(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, const aton_params_t *params,
+                       void *cuda_stream, bool slab, int z_begin, int nz_local) {
     if (out) *out = nullptr;
     if (!out || !grid || !box || !params) return fail(nullptr, ATON_EINVAL, "aton_init: NULL argument");
     if (grid->nx < 4 || grid->nx % 4 != 0 || grid->ny < 1 || grid->nz < 1)
         return fail(nullptr, ATON_EINVAL, "aton_init: need nx %% 4 == 0, nx >= 4, ny, nz >= 1 (got %d %d %d)",
                     grid->nx, grid->ny, grid->nz);
-    const double ncell_d = (double)grid->nx * grid->ny * grid->nz;
-    if (ncell_d >= 2147483648.0) return fail(nullptr, ATON_EINVAL, "aton_init: nx*ny*nz must be < 2^31");
+    if (slab && (z_begin < 0 || nz_local < 1 || z_begin + nz_local > grid->nz))
+        return fail(nullptr, ATON_EINVAL, "aton_init_slab: planes [%d, %d) are not inside nz = %d", z_begin,
+                    z_begin + nz_local, grid->nz);
+    if (slab && !v4_grid_ok(Grid{grid->nx, grid->ny, nz_local + 2}))
+        return fail(nullptr, ATON_EINVAL, "aton_init_slab: needs nx %% 32 == 0 and ny %% 4 == 0 (kernel variant 4)");
+    const int nz_own = slab ? nz_local : grid->nz, nz_alloc = slab ? nz_local + 2 : grid->nz;
+    const double nalloc_d = (double)grid->nx * grid->ny * nz_alloc;
+    if (nalloc_d >= 2147483648.0) return fail(nullptr, ATON_EINVAL, "aton_init: nx*ny*nz must be < 2^31");
     if (!(box->lx_cm > 0.0)) return fail(nullptr, ATON_EINVAL, "aton_init: lx_cm must be > 0");
     if (!(params->sigma_n > 0.0) || !(params->sigma_e > 0.0) || !(params->e_photon_eV > 0.0))
         return fail(nullptr, ATON_EINVAL, "aton_init: sigma_n, sigma_e, e_photon_eV must be > 0");
@@ -246,29 +260,37 @@ int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, cons
     }
     aton_ctx *ctx = new (std::nothrow) aton_ctx();
     if (!ctx) return fail(nullptr, ATON_ENOMEM, "aton_init: host allocation failed");
-    ctx->g = Grid{grid->nx, grid->ny, grid->nz};
-    ctx->ncell = (size_t)ncell_d;
+    ctx->g = Grid{grid->nx, grid->ny, nz_alloc};
+    ctx->plane = (size_t)grid->nx * grid->ny;
+    ctx->ncell = ctx->plane * nz_own;
+    ctx->nalloc = (size_t)nalloc_d;
+    ctx->slab = slab;
+    ctx->off = slab ? ctx->plane : 0;
+    ctx->z_begin = slab ? z_begin : 0;
+    ctx->nz_local = nz_own;
+    ctx->nz_global = grid->nz;
     ctx->p = *params;
     ctx->c = params->c_cm_s > 0.0 ? params->c_cm_s : 2.99792458e10;
     if (ctx->p.eps_sub == 0.0) ctx->p.eps_sub = 0.1;
     if (ctx->p.max_sub == 0) ctx->p.max_sub = 1 << 14;
     ctx->dx = box->lx_cm / grid->nx;
     ctx->stream = (cudaStream_t)cuda_stream;
-    const size_t bytes = ctx->ncell * sizeof(float);
+    const size_t bytes = ctx->nalloc * sizeof(float);
     cudaError_t e = cudaSuccess;
     float **slots[11] = {&ctx->rad[0][0], &ctx->rad[0][1], &ctx->rad[0][2], &ctx->rad[0][3], &ctx->rad[1][0],
                          &ctx->rad[1][1], &ctx->rad[1][2], &ctx->rad[1][3], &ctx->x, &ctx->T, &ctx->nH};
     for (int i = 0; i < 11 && e == cudaSuccess; i++) e = cudaMalloc((void **)slots[i], bytes);
+    for (int i = 0; i < 11 && e == cudaSuccess && slab; i++) e = cudaMemsetAsync(*slots[i], 0, bytes, ctx->stream);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, 3 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->partials, sizeof(double) * (REDUCE_BLOCKS + 1) * R_COUNT);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_mask, sizeof(unsigned) * (ctx->ncell / 1024 + 1));
-    const size_t defer_bytes = sizeof(unsigned) * (ctx->ncell / 32 + 1);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_mask, sizeof(unsigned) * (ctx->nalloc / 1024 + 1));
+    const size_t defer_bytes = sizeof(unsigned) * (ctx->nalloc / 32 + 1);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->defer_mask, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->defer_mask, 0, defer_bytes, ctx->stream);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_bits, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_bits, 0, defer_bytes, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->ncell / 1024 + 1), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->nalloc / 1024 + 1), ctx->stream);
     if (e != cudaSuccess) {
         int code = fail(nullptr, e == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,
                         "aton_init: device allocation failed: %s", cudaGetErrorString(e));
@@ -278,6 +300,16 @@ int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, cons
     }
     *out = ctx;
     return ATON_OK;
+}
+
+int aton_init(aton_t **out, const aton_grid_t *grid, const aton_box_t *box, const aton_params_t *params,
+              void *cuda_stream) {
+    return init_common(out, grid, box, params, cuda_stream, false, 0, 0);
+}
+
+int aton_init_slab(aton_t **out, const aton_grid_t *global_grid, const aton_box_t *box, const aton_params_t *params,
+                   void *cuda_stream, int z_begin, int nz_local) {
+    return init_common(out, global_grid, box, params, cuda_stream, true, z_begin, nz_local);
 }
 
 void aton_free(aton_t *ctx) {
@@ -335,13 +367,15 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     ctx->have_fields = false;
     ctx->cur = 0;
-    CU(ctx, cudaMemcpyAsync(ctx->nH, nH, bytes, kind, ctx->stream));
-    CU(ctx, cudaMemcpyAsync(ctx->x, x, bytes, kind, ctx->stream));
-    CU(ctx, cudaMemcpyAsync(ctx->T, T, bytes, kind, ctx->stream));
+    const size_t o = ctx->off;             // a slab's own planes start one (ghost) plane in
+    CU(ctx, cudaMemcpyAsync(ctx->nH + o, nH, bytes, kind, ctx->stream));
+    CU(ctx, cudaMemcpyAsync(ctx->x + o, x, bytes, kind, ctx->stream));
+    CU(ctx, cudaMemcpyAsync(ctx->T + o, T, bytes, kind, ctx->stream));
     const float *rad_in[4] = {N, Fx, Fy, Fz};
     const float inv_c = (float)(1.0 / ctx->c);
     for (int v = 0; v < 4; v++) {
-        float *dst = ctx->rad[0][v];
+        float *dst = ctx->rad[0][v] + o;
+        if (ctx->slab) CU(ctx, cudaMemsetAsync(ctx->rad[0][v], 0, ctx->nalloc * sizeof(float), ctx->stream));
         if (!rad_in[v]) {
             CU(ctx, cudaMemsetAsync(dst, 0, bytes, ctx->stream));
         } else {
@@ -358,7 +392,7 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
     if (rc) return rc;
     if (!(red[R_NHMIN] > 0.0) || !std::isfinite(red[R_M]))
         return fail(ctx, ATON_EINVAL, "aton_set_fields: n_H must be finite and > 0 everywhere (min %g)", red[R_NHMIN]);
-    ctx->nH_mean = red[R_M] / (double)ctx->ncell;
+    if (!ctx->mean_set) ctx->nH_mean = red[R_M] / (double)ctx->ncell;
     ctx->steps_done = 0;
     ctx->fast_subcycles = 0;
     ctx->time_s = 0.0;
@@ -379,8 +413,9 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
         pos = hpos.data(); rate = hrate.data();
     }
     // NGP binning: cell = floor(pos*n) mod n; merge sources sharing a cell (fp64)
-    std::vector<std::pair<int, double>> cells((size_t)n);
-    const int dims[3] = {ctx->g.nx, ctx->g.ny, ctx->g.nz};
+    std::vector<std::pair<int, double>> cells;
+    cells.reserve((size_t)n);
+    const int dims[3] = {ctx->g.nx, ctx->g.ny, ctx->nz_global};     // positions refer to the global box
     for (long long s = 0; s < n; s++) {
         int ijk[3];
         for (int a = 0; a < 3; a++) {
@@ -391,7 +426,12 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
         }
         if (!(rate[s] >= 0.0) || !std::isfinite(rate[s]))
             return fail(ctx, ATON_EINVAL, "aton_set_sources: rate %lld must be finite and >= 0", s);
-        cells[s] = {ijk[0] + ctx->g.nx * (ijk[1] + ctx->g.ny * ijk[2]), rate[s]};
+        int k = ijk[2];
+        if (ctx->slab) {       // keep the sources of this slab; local plane index counts the ghost plane below
+            if (k < ctx->z_begin || k >= ctx->z_begin + ctx->nz_local) continue;
+            k = k - ctx->z_begin + 1;
+        }
+        cells.push_back({ijk[0] + ctx->g.nx * (ijk[1] + ctx->g.ny * k), rate[s]});
     }
     std::stable_sort(cells.begin(), cells.end(), [](const auto &a, const auto &b) { return a.first < b.first; });
     std::vector<int> ucell;
@@ -401,7 +441,7 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
         else { ucell.push_back(cr.first); urate.push_back(cr.second); }
     }
     const size_t nu = ucell.size();
-    const size_t nwords = ctx->ncell / 1024 + 1;
+    const size_t nwords = ctx->nalloc / 1024 + 1;
     std::vector<unsigned> mask(nwords, 0u);
     std::vector<float> rho(nu);
     const double inv_vol = 1.0 / (ctx->dx * ctx->dx * ctx->dx);
@@ -414,7 +454,7 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
     cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
     ctx->src_cell = nullptr; ctx->src_rho = nullptr; ctx->n_src = 0;
     CU(ctx, cudaMemcpyAsync(ctx->src_mask, mask.data(), sizeof(unsigned) * nwords, cudaMemcpyHostToDevice, ctx->stream));
-    CU(ctx, cudaMemsetAsync(ctx->src_bits, 0, sizeof(unsigned) * (ctx->ncell / 32 + 1), ctx->stream));
+    CU(ctx, cudaMemsetAsync(ctx->src_bits, 0, sizeof(unsigned) * (ctx->nalloc / 32 + 1), ctx->stream));
     if (nu > 0) {
         CU(ctx, cudaMalloc((void **)&ctx->src_cell, sizeof(int) * nu));
         CU(ctx, cudaMalloc((void **)&ctx->src_rho, sizeof(float) * nu));
@@ -442,6 +482,10 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     const double mu = ctx->c * dt / ctx->dx;
     if (!(mu <= (1.0 / 3.0) * (1.0 + 1e-12)) || !std::isfinite(mu))
         return fail(ctx, ATON_EINVAL, "aton_step: c*dt/dx = %g > 1/3 is unstable for the unsplit 3-D LF scheme", mu);
+    if (ctx->slab && ctx->variant != 4)
+        return fail(ctx, ATON_ESTATE, "aton_step: a slab context runs kernel variant 4 only");
+    if (ctx->slab && n_steps > 1)
+        return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first)");
     const StepConst sc = make_step_const(ctx, dt);
     for (int s = 0; s < n_steps; s++) {
         CU(ctx, launch_step(ctx, sc));
@@ -452,25 +496,81 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     return ATON_OK;
 }
 
+int aton_set_mean_density(aton_t *ctx, double nH_mean) {
+    if (!ctx) return ATON_EINVAL;
+    if (!(nH_mean > 0.0) || !std::isfinite(nH_mean)) return fail(ctx, ATON_EINVAL, "aton_set_mean_density: must be > 0");
+    ctx->nH_mean = nH_mean;
+    ctx->mean_set = true;
+    return ATON_OK;
+}
+
+// halo planes of a slab: [4 fields][ny][nx] each, fields in the order N, Gx, Gy, Gz (G = F/c, as carried)
+int aton_halo_pack(aton_t *ctx, float *send_lo, float *send_hi) {
+    if (!ctx || !send_lo || !send_hi) return ATON_EINVAL;
+    if (!ctx->slab) return fail(ctx, ATON_ESTATE, "aton_halo_pack: not a slab context");
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_halo_pack: no fields set");
+    const size_t pb = ctx->plane * sizeof(float);
+    for (int v = 0; v < 4; v++) {
+        const float *a = ctx->rad[ctx->cur][v];
+        CU(ctx, cudaMemcpyAsync(send_lo + v * ctx->plane, a + ctx->plane, pb, cudaMemcpyDeviceToDevice, ctx->stream));
+        CU(ctx, cudaMemcpyAsync(send_hi + v * ctx->plane, a + (size_t)ctx->nz_local * ctx->plane, pb,
+                                cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    return ATON_OK;
+}
+
+int aton_halo_unpack(aton_t *ctx, const float *recv_lo, const float *recv_hi) {
+    if (!ctx || !recv_lo || !recv_hi) return ATON_EINVAL;
+    if (!ctx->slab) return fail(ctx, ATON_ESTATE, "aton_halo_unpack: not a slab context");
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_halo_unpack: no fields set");
+    const size_t pb = ctx->plane * sizeof(float);
+    for (int v = 0; v < 4; v++) {
+        float *a = ctx->rad[ctx->cur][v];
+        CU(ctx, cudaMemcpyAsync(a, recv_lo + v * ctx->plane, pb, cudaMemcpyDeviceToDevice, ctx->stream));
+        CU(ctx, cudaMemcpyAsync(a + (size_t)(ctx->nz_local + 1) * ctx->plane, recv_hi + v * ctx->plane, pb,
+                                cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    return ATON_OK;
+}
+
+int aton_reduce_sums(aton_t *ctx, double *sums, int n) {
+    if (!ctx || !sums) return ATON_EINVAL;
+    if (n != ATON_NSUMS) return fail(ctx, ATON_EINVAL, "aton_reduce_sums: n must be ATON_NSUMS (%d)", ATON_NSUMS);
+    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_reduce_sums: no fields set");
+    double r[R_COUNT];
+    int rc = run_reduce(ctx, true, r);
+    if (rc) return rc;
+    unsigned long long st[3];
+    CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    sums[0] = (double)ctx->ncell; sums[1] = r[R_X]; sums[2] = r[R_XM]; sums[3] = r[R_M]; sums[4] = r[R_N];
+    sums[5] = r[R_NM]; sums[6] = r[R_T]; sums[7] = r[R_HALF]; sums[8] = r[R_BAD];
+    sums[9] = (double)((long long)st[0] + ctx->fast_subcycles); sums[10] = (double)st[2];
+    sums[11] = std::sqrt(r[R_F2MAX]); sums[12] = (double)std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
+    sums[13] = r[R_NMIN];
+    return ATON_OK;
+}
+
 int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float *Fx, float *Fy, float *Fz,
                     int on_device) {
     if (!ctx) return ATON_EINVAL;
     if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_get_fields: no fields set");
     const size_t bytes = ctx->ncell * sizeof(float);
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
-    if (nH) CU(ctx, cudaMemcpyAsync(nH, ctx->nH, bytes, kind, ctx->stream));
-    if (x) CU(ctx, cudaMemcpyAsync(x, ctx->x, bytes, kind, ctx->stream));
-    if (T) CU(ctx, cudaMemcpyAsync(T, ctx->T, bytes, kind, ctx->stream));
-    if (N) CU(ctx, cudaMemcpyAsync(N, ctx->rad[ctx->cur][0], bytes, kind, ctx->stream));
+    const size_t o = ctx->off;
+    if (nH) CU(ctx, cudaMemcpyAsync(nH, ctx->nH + o, bytes, kind, ctx->stream));
+    if (x) CU(ctx, cudaMemcpyAsync(x, ctx->x + o, bytes, kind, ctx->stream));
+    if (T) CU(ctx, cudaMemcpyAsync(T, ctx->T + o, bytes, kind, ctx->stream));
+    if (N) CU(ctx, cudaMemcpyAsync(N, ctx->rad[ctx->cur][0] + o, bytes, kind, ctx->stream));
     float *outs[3] = {Fx, Fy, Fz};
     for (int v = 0; v < 3; v++) {
         if (!outs[v]) continue;
-        const float *G = ctx->rad[ctx->cur][1 + v];
+        const float *G = ctx->rad[ctx->cur][1 + v] + o;
         if (on_device) {
             int rc = scale_into(ctx, G, outs[v], (float)ctx->c);
             if (rc) return rc;
         } else {   // F = c G staged in the idle ping-pong buffer
-            float *stage = ctx->rad[1 - ctx->cur][1 + v];
+            float *stage = ctx->rad[1 - ctx->cur][1 + v] + o;
             int rc = scale_into(ctx, G, stage, (float)ctx->c);
             if (rc) return rc;
             CU(ctx, cudaMemcpyAsync(outs[v], stage, bytes, kind, ctx->stream));

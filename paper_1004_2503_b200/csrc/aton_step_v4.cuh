@@ -68,7 +68,7 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
 #endif
 template <int FLAGS>
 __global__ void __launch_bounds__(V4Cfg::THREADS, ATON_V4_MINB)
-step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
+step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     using C = V4Cfg;
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -79,8 +79,10 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
     float *wyp = raw + 2 * C::RAW_BUF;                   // [4][4][32] plus terms
     float *wym = wyp + C::W_SIGN;                        //            minus terms
 
-    const int x0 = xt * C::WX, y0 = blockIdx.y * C::WY, z0 = blockIdx.z * lz;
-    const int lzn = min(lz, g.nz - z0);
+    // planes [zb, ze) are advanced: the whole periodic grid (0, nz), or a slab's own planes (1, nz - 1) whose
+    // ghost planes 0 and nz - 1 hold the neighbours' boundary planes (no wrap is ever taken then)
+    const int x0 = xt * C::WX, y0 = blockIdx.y * C::WY, z0 = zb + blockIdx.z * lz;
+    const int lzn = min(lz, ze - z0);
     const int plane = g.nx * g.ny;
     const int rowoff = (y0 + r) * g.nx + x0 + 4 * q;     // own quad inside a plane
     // y halo row of this lane: rows 0 / 3 take the row below / above the tile (others: a harmless re-read)
@@ -327,16 +329,17 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
 
 inline bool v4_grid_ok(const Grid &g) { return g.nx % V4Cfg::WX == 0 && g.ny % V4Cfg::WY == 0; }
 
-inline int v4_default_lz(const Grid &g, int tile_z) {
-    if (tile_z > 0) return tile_z < g.nz ? tile_z : g.nz;
+inline int v4_default_lz(const Grid &g, int tile_z, int nzr) {
+    if (tile_z > 0) return tile_z < nzr ? tile_z : nzr;
     const long tiles_xy = (long)((g.nx / V4Cfg::WX + V4Cfg::WARPS - 1) / V4Cfg::WARPS) * (g.ny / V4Cfg::WY);
     int lz = 64;      // largest power of two <= 64 that still gives >= 4 waves of 4 CTAs per SM
-    while (lz > 4 && tiles_xy * ((g.nz + lz - 1) / lz) < 16L * 148) lz >>= 1;
-    return lz < g.nz ? lz : g.nz;
+    while (lz > 4 && tiles_xy * ((nzr + lz - 1) / lz) < 16L * 148) lz >>= 1;
+    return lz < nzr ? lz : nzr;
 }
 
 template <int FLAGS>
-cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream) {
+cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream,
+                           int zb, int ze) {
     using C = V4Cfg;
     static bool attr_done = false;     // one per instantiation
     if (!attr_done) {
@@ -344,9 +347,9 @@ cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c,
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int lz = v4_default_lz(g, tile_z);
-    const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (g.nz + lz - 1) / lz);
-    step_v4_kernel<FLAGS><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz);
+    const int lz = v4_default_lz(g, tile_z, ze - zb);
+    const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (ze - zb + lz - 1) / lz);
+    step_v4_kernel<FLAGS><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz, zb, ze);
     return cudaGetLastError();
 }
 
