@@ -180,14 +180,26 @@ def run_ours(args, rank, world, local_rank):
     w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
     if args.state == "warm":
         w = wl.synthetic_warm_state(w)
-    a = aton.from_workload(w)
     variant = 4 if args.variant is None else args.variant
-    a.set_kernel(variant, args.tile_y, args.tile_z)
+    if args.decomp == "slab":
+        # ONE box of n x n x (n * world) cells cut into z slabs, one per rank, halo planes exchanged every step
+        # (NEXT-1); each rank generates its own n^3 part of the density and its sources
+        from paper_1004_2503_b200 import slab
+        sl = slab.SlabAton(n, n, n * world, w.box_cm, w.params, rank, world)
+        sl.set_fields(w.nH, w.x, w.T, w.N, w.Fx, w.Fy, w.Fz)
+        pos = w.src_pos.clone()
+        pos[:, 2] = (pos[:, 2] + rank) / world
+        sl.set_sources(pos.contiguous(), w.src_rate.contiguous())
+        a, do_step = sl.ctx, sl.step
+    else:
+        a = aton.from_workload(w)
+        a.set_kernel(variant, args.tile_y, args.tile_z)
+        do_step = a.step
     cells = float(n) ** 3
     stream = torch.cuda.current_stream()
 
     # ---- device-resident timing: inputs already in HBM, aton_step only
-    a.step(w.dt, args.warmup)
+    do_step(w.dt, args.warmup)
     torch.cuda.synchronize()
     if world > 1:
         torch.distributed.barrier()
@@ -196,7 +208,7 @@ def run_ours(args, rank, world, local_rank):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record(stream)
-    a.step(w.dt, args.steps)
+    do_step(w.dt, args.steps)
     e1.record(stream)
     torch.cuda.synchronize()
     if world > 1:
@@ -210,7 +222,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- the dominant kernel alone: CUDA events on the library's stream around each of its launches
     #      (aton_set_timing), in a second pass of the same K steps so the events stay out of `value`
     a.set_timing(True)
-    a.step(w.dt, args.steps)
+    do_step(w.dt, args.steps)
     k_ms_total, k_n = a.kernel_time()
     a.set_timing(False)
     kernel_ms = k_ms_total / max(k_n, 1)
@@ -228,7 +240,7 @@ def run_ours(args, rank, world, local_rank):
             torch.distributed.barrier()
         t0 = time.perf_counter()
         a.set_fields(host["nH"], host["x"], host["T"])            # dark start: N, F = NULL
-        a.step(w.dt, args.steps)
+        do_step(w.dt, args.steps)
         a.get_fields(out=out)                                      # synchronises
         t_e2e = (time.perf_counter() - t0) * 1e3
         if world > 1:
@@ -262,7 +274,8 @@ def run_ours(args, rank, world, local_rank):
                                    f"physics flags {dict((k, w.params[k]) for k in ('recomb_case', 'cooling', 'coll_ion', 'clump_model'))}",
                        "state": args.state + f" start + {args.warmup} warm-up steps",
                        "l2": "working set per step (52 B/cell) exceeds the 126 MB L2" if 52 * cells > 4 * 126e6 else "fits in L2 (latency bound; not an HBM figure)",
-                       "parallelism": "replicas" if world > 1 else "single GPU",
+                       "parallelism": ("z slabs of one box, halo planes exchanged every step" if args.decomp == "slab"
+                                       else "replicas" if world > 1 else "single GPU"),
                        "x_vol_end": diag["x_vol"], "subcycles_per_cell_step": diag["subcycles_total"] / cells / max(diag["steps_done"], 1),
                        "subcycles_max": diag["subcycles_max"], "n_nonfinite": diag["n_nonfinite"]},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks}
@@ -278,6 +291,8 @@ def main():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--n", type=int, default=None, help="grid size override (down-sized twin)")
     ap.add_argument("--state", default="dark", choices=["dark", "warm"])
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, the north_star's single-GPU path) or z slabs of one box")
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--tile-y", type=int, default=0)
     ap.add_argument("--tile-z", type=int, default=0)
