@@ -121,9 +121,10 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out);
  * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel;
  * 3 = variant 2's arithmetic with full CTA tiles and a split-phase barrier (nx % 128 == 0, ny % tile_y == 0);
  * 4 (default) = warp-autonomous tiles, no inter-warp synchronisation, sources injected by the fix-up
- * kernel (nx % 32 == 0, ny % 4 == 0).  A grid a variant cannot tile runs the variant-2 kernel.
+ * kernel (nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0 and ny % 2 == 0).  A grid a variant cannot tile runs the
+ * variant-2 kernel.
  * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6;
- * variant 3: tile_y in {4, 8, 16}, default 8; variant 4: tile_y must be 0; tile_z = planes per z-chunk);
+ * variant 3: tile_y in {4, 8, 16}, default 8; variant 4: tile_y 4 = 32 x 4 warp tiles (default), 2 = 64 x 2; tile_z = planes per z-chunk);
  * results agree between variants to rounding and do not depend on the tile shape.  ATON_EINVAL otherwise. */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 

@@ -164,13 +164,14 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
     }
     // variant 4 needs nx % 32 == 0, ny % 4 == 0; variant 3 nx % 128 == 0, ny % TY == 0; other grids run the
     // variant-2 kernel.  Only variant 4 leaves the source injection to the fix-up kernel.
-    const bool use4 = ctx->variant == 4 && v4_grid_ok(ctx->g);
+    const int wxq4 = ctx->variant == 4 ? v4_pick_wxq(ctx->g, ctx->tile_y) : 0;
+    const bool use4 = wxq4 != 0;
     if (ctx->slab && !use4) return cudaErrorNotSupported;    // checked with a message in aton_step
     const int ty3 = ctx->variant == 3 ? v3_pick_ty(ctx->g, ctx->tile_y) : 0;
     FieldsIO f2 = f;
     f2.fix_inject = use4 ? 1 : 0;
     time_mark(ctx);
-    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
+    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, wxq4, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
                                                  ctx->slab ? ctx->nz_local + 1 : ctx->g.nz)
                     : ty3 ? launch_step_v3<FLAGS>(f2, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
                           : launch_step_fused<FLAGS>(f2, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0,
@@ -331,7 +332,7 @@ int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
     if (variant < 0 || variant > 4) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0..4");
     if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)) ||
-        (variant == 3 && !v3_shape_ok(tile_y, tile_z)) || (variant == 4 && (tile_y != 0 || tile_z < 0)))
+        (variant == 3 && !v3_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     return ATON_OK;

@@ -1,4 +1,5 @@
-// Fused step kernel, variant 4 (the product kernel for grids with nx % 32 == 0 and ny % 4 == 0):
+// Fused step kernel, variant 4 (the product kernel for grids with nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0
+// and ny % 2 == 0; the comments below describe the default 32 x 4 tile, WXQ = 8):
 // WARP-AUTONOMOUS tiles.  Transport + one chemistry sub-step in one pass over HBM (52 B per cell-update);
 // source cells and cells that need sub-cycling go to step_fixup_kernel.
 //
@@ -30,13 +31,15 @@ namespace aton {
 #ifndef ATON_V4_WARPS
 #define ATON_V4_WARPS 4
 #endif
+// WXQ = quads per tile row: 8 -> a 32 x 4 tile (the default), 16 -> 64 x 2
+template <int WXQ>
 struct V4Cfg {
-    static constexpr int WX = 32, WY = 4;                // cells per warp tile
-    static constexpr int RS = 40;                        // raw row: quads at col 4 + 4q, x halos at 3 and 36
+    static constexpr int WX = 4 * WXQ, WY = 32 / WXQ;    // cells per warp tile
+    static constexpr int RS = WX + 8;                    // raw row: quads at col 4 + 4q, x halos at 3 and 4 + WX
     static constexpr int RAW_FIELD = (WY + 2) * RS;      // row slots 0 / WY+1 = y halo rows
     static constexpr int RAW_BUF = 4 * RAW_FIELD;        // [field][slot][RS]
     static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
-    static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][32]
+    static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][WX]
     static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN;
     static constexpr int WARPS = ATON_V4_WARPS, THREADS = 32 * WARPS;
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
@@ -66,13 +69,13 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
 #ifndef ATON_V4_MINB
 #define ATON_V4_MINB 4
 #endif
-template <int FLAGS>
-__global__ void __launch_bounds__(V4Cfg::THREADS, ATON_V4_MINB)
+template <int FLAGS, int WXQ>
+__global__ void __launch_bounds__(V4Cfg<WXQ>::THREADS, ATON_V4_MINB)
 step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
-    using C = V4Cfg;
+    using C = V4Cfg<WXQ>;
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int r = lane >> 3, q = lane & 7;
+    const int r = lane / WXQ, q = lane % WXQ;
     const int xt = blockIdx.x * C::WARPS + warp;         // x tile of this warp
     if (xt * C::WX >= g.nx) return;                      // ragged last CTA in x: warps are independent
     float *raw = smem + warp * C::WARP_FLOATS;           // [2][4][6][RS], thread-private entries
@@ -91,12 +94,12 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     const int hoff = jh * g.nx + x0 + 4 * q;
     const int hslot = hbot ? 0 : (htop ? C::WY + 1 : r + 1);
     // x halo cell of this lane: q = 0 the cell left of the tile, q = 7 the cell right of it
-    const bool edge_l = q == 0, edge_r = q == 7;
+    const bool edge_l = q == 0, edge_r = q == WXQ - 1;
     const int xh = edge_l ? (x0 == 0 ? g.nx - 1 : x0 - 1) : (x0 + C::WX == g.nx ? 0 : x0 + C::WX);
     const int xoff = (y0 + r) * g.nx + xh;
     const int my = (r + 1) * C::RS + 4 + 4 * q;          // own quad inside a raw field
     const int myh = hslot * C::RS + 4 + 4 * q;           // halo-row quad
-    const int mxh = (r + 1) * C::RS + (edge_l ? 3 : 36); // x halo cell (valid for edge lanes)
+    const int mxh = (r + 1) * C::RS + (edge_l ? 3 : 4 + C::WX); // x halo cell (valid for edge lanes)
     const float *src[4] = {f.N, f.Gx, f.Gy, f.Gz};
 
     int kst = z0 == 0 ? g.nz - 1 : z0 - 1;               // plane index staged next (periodic)
@@ -182,14 +185,14 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
                     const f2 p0 = u.v[0][v] + F[0][v], p1 = u.v[1][v] + F[1][v];
                     const f2 m0 = u.v[0][v] - F[0][v], m1 = u.v[1][v] - F[1][v];
 #if ATON_V4_X & 2
-                    sts128_if(wyp + v * C::W_COMP + (r + 1) * 32 + 4 * q, lo(p0), hi(p0), lo(p1), hi(p1), !htop);
-                    sts128_if(wym + v * C::W_COMP + (r - 1) * 32 + 4 * q, lo(m0), hi(m0), lo(m1), hi(m1), !hbot);
+                    sts128_if(wyp + v * C::W_COMP + (r + 1) * C::WX + 4 * q, lo(p0), hi(p0), lo(p1), hi(p1), !htop);
+                    sts128_if(wym + v * C::W_COMP + (r - 1) * C::WX + 4 * q, lo(m0), hi(m0), lo(m1), hi(m1), !hbot);
 #else
                     if (!htop)
-                        *reinterpret_cast<float4 *>(wyp + v * C::W_COMP + (r + 1) * 32 + 4 * q) =
+                        *reinterpret_cast<float4 *>(wyp + v * C::W_COMP + (r + 1) * C::WX + 4 * q) =
                             make_float4(lo(p0), hi(p0), lo(p1), hi(p1));
                     if (!hbot)
-                        *reinterpret_cast<float4 *>(wym + v * C::W_COMP + (r - 1) * 32 + 4 * q) =
+                        *reinterpret_cast<float4 *>(wym + v * C::W_COMP + (r - 1) * C::WX + 4 * q) =
                             make_float4(lo(m0), hi(m0), lo(m1), hi(m1));
 #endif
                 }
@@ -211,7 +214,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
 #pragma unroll
                     for (int v = 0; v < 4; v++) w[p][v] = fma2(F[v], sg, e[v]);
                 }
-                float *wdst = hbot ? wyp + 4 * q : wym + (C::WY - 1) * 32 + 4 * q;
+                float *wdst = hbot ? wyp + 4 * q : wym + (C::WY - 1) * C::WX + 4 * q;
 #if ATON_V4_X & 2
 #pragma unroll
                 for (int v = 0; v < 4; v++)
@@ -265,7 +268,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
                 float right = __shfl_down_sync(0xffffffffu, lo(Wm[0][v]), 1);
 #if ATON_V4_X & 1
                 left = slct(left, lo(eWp[v]), q - 1);         // q == 0: the halo cell
-                right = slct(right, lo(eWm[v]), 6 - q);       // q == 7: the halo cell
+                right = slct(right, lo(eWm[v]), WXQ - 2 - q); // q == WXQ - 1: the halo cell
 #else
                 left = edge_l ? lo(eWp[v]) : left;
                 right = edge_r ? lo(eWm[v]) : right;
@@ -300,7 +303,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         }
         // ---- y terms of plane m, written straight into the carried registers
         if (INPL) {
-            const int rp = r * 32 + 4 * q;
+            const int rp = r * C::WX + 4 * q;
 #pragma unroll
             for (int v = 0; v < 4; v++) {
                 const float4 yp = *reinterpret_cast<const float4 *>(wyp + v * C::W_COMP + rp);
@@ -327,30 +330,51 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     iter(no, yes, false, false);               // m = lzn + 1: z halo plane above, finishes plane lzn
 }
 
-inline bool v4_grid_ok(const Grid &g) { return g.nx % V4Cfg::WX == 0 && g.ny % V4Cfg::WY == 0; }
+// tile shapes: 32 x 4 (nx % 32 == 0, ny % 4 == 0; the default: 13.8 ms per 1024^3 step) or 64 x 2 (nx % 64 == 0,
+// ny % 2 == 0; 14.1 ms: its 256-byte row segments stream better in isolation, but every row is then read twice
+// and the tile halo costs more than the segments gain -- profiles/r01_e_tile_shape.md).  `tile_y` = 4 / 2 forces
+// one, 0 picks 32 x 4 when the grid allows it.  Results do not depend on the shape (bitwise).  Returns WXQ or 0.
+inline int v4_pick_wxq(const Grid &g, int tile_y) {
+    const bool ok16 = g.nx % 64 == 0 && g.ny % 2 == 0, ok8 = g.nx % 32 == 0 && g.ny % 4 == 0;
+    if (tile_y == 2) return ok16 ? 16 : 0;
+    if (tile_y == 4) return ok8 ? 8 : 0;
+    return ok8 ? 8 : (ok16 ? 16 : 0);
+}
+inline bool v4_grid_ok(const Grid &g) { return v4_pick_wxq(g, 0) != 0; }
+inline bool v4_shape_ok(int tile_y, int tile_z) { return (tile_y == 0 || tile_y == 2 || tile_y == 4) && tile_z >= 0; }
 
+template <int WXQ>
 inline int v4_default_lz(const Grid &g, int tile_z, int nzr) {
+    using C = V4Cfg<WXQ>;
     if (tile_z > 0) return tile_z < nzr ? tile_z : nzr;
-    const long tiles_xy = (long)((g.nx / V4Cfg::WX + V4Cfg::WARPS - 1) / V4Cfg::WARPS) * (g.ny / V4Cfg::WY);
+    const long tiles_xy = (long)((g.nx / C::WX + C::WARPS - 1) / C::WARPS) * (g.ny / C::WY);
     int lz = 64;      // largest power of two <= 64 that still gives >= 4 waves of 4 CTAs per SM
     while (lz > 4 && tiles_xy * ((nzr + lz - 1) / lz) < 16L * 148) lz >>= 1;
     return lz < nzr ? lz : nzr;
 }
 
-template <int FLAGS>
-cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream,
-                           int zb, int ze) {
-    using C = V4Cfg;
+template <int FLAGS, int WXQ>
+cudaError_t launch_step_v4_wxq(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream,
+                               int zb, int ze) {
+    using C = V4Cfg<WXQ>;
     static bool attr_done = false;     // one per instantiation
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS, WXQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int lz = v4_default_lz(g, tile_z, ze - zb);
+    const int lz = v4_default_lz<WXQ>(g, tile_z, ze - zb);
     const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (ze - zb + lz - 1) / lz);
-    step_v4_kernel<FLAGS><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz, zb, ze);
+    step_v4_kernel<FLAGS, WXQ><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz, zb, ze);
     return cudaGetLastError();
+}
+
+// wxq must come from v4_pick_wxq (non-zero)
+template <int FLAGS>
+cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int wxq, int tile_z, cudaStream_t stream,
+                           int zb, int ze) {
+    if (wxq == 8) return launch_step_v4_wxq<FLAGS, 8>(f, g, c, tile_z, stream, zb, ze);
+    return launch_step_v4_wxq<FLAGS, 16>(f, g, c, tile_z, stream, zb, ze);
 }
 
 }  // namespace aton
