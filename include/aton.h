@@ -143,7 +143,7 @@ int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches);
  * re-cut as z slabs whose one-plane halo of (N, F) is one contiguous block per field) ----
  *
  * aton_init_slab creates a context that advances planes [z_begin, z_begin + nz_local) of the GLOBAL grid
- * `global_grid` (needs nx % 32 == 0, ny % 4 == 0: kernel variant 4).  It holds nz_local + 2 planes per array: its
+ * `global_grid` (needs a grid kernel variant 4 can tile: nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0 and ny % 2 == 0).  It holds nz_local + 2 planes per array: its
  * own planes between a ghost plane below and one above.  aton_set_fields / aton_get_fields then take arrays of
  * nz_local planes; aton_set_sources takes positions in the GLOBAL box and keeps the sources of the slab;
  * aton_reduce reports the slab's own means.  Before EVERY aton_step(ctx, dt, 1) the caller exchanges halos:
