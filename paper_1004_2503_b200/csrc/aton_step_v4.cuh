@@ -58,7 +58,25 @@ __device__ __forceinline__ void sts128_if(float *p, float a, float b, float c, f
     asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %5, 0;\n@p st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n}"
                  ::"r"(smem_u32(p)), "f"(a), "f"(b), "f"(c), "f"(d), "r"(pred) : "memory");
 }
+#ifndef ATON_V4_CS
+#define ATON_V4_CS 0     // bit 0: streaming loads of x, T, n_H; bit 1: streaming stores
+#endif
+#ifndef ATON_V4_CA
+#define ATON_V4_CA 1     // 1: stage quads through L1 (cp.async.ca) so that a neighbour tile's halo request can hit there
+#endif
+__device__ __forceinline__ void cp_async16_own(void *smem, const void *gmem) {
+#if ATON_V4_CA
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+#else
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+#endif
+}
 __device__ __forceinline__ void cp_async16_if(void *smem, const void *gmem, int pred) {
+#if ATON_V4_CA
+    asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %2, 0;\n@p cp.async.ca.shared.global [%0], [%1], 16;\n}"
+                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(pred) : "memory");
+    return;
+#endif
     asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %2, 0;\n@p cp.async.cg.shared.global [%0], [%1], 16;\n}"
                  ::"r"(smem_u32(smem)), "l"(gmem), "r"(pred) : "memory");
 }
@@ -107,7 +125,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         float *dst = raw + (m & 1) * C::RAW_BUF;
         const int base = kst * plane;
 #pragma unroll
-        for (int v = 0; v < 4; v++) cp_async16(dst + v * C::RAW_FIELD + my, src[v] + base + rowoff);
+        for (int v = 0; v < 4; v++) cp_async16_own(dst + v * C::RAW_FIELD + my, src[v] + base + rowoff);
         if (inpl) {
 #if ATON_V4_X & 4
 #pragma unroll
@@ -152,9 +170,15 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), T4 = x4, h4 = make_float4(1.f, 1.f, 1.f, 1.f);
         unsigned srcw = 0;
         if (FIN) {
+#if ATON_V4_CS & 1       // read once: streaming loads keep the (N, G) rows that tile halos re-read in L2
+            x4 = __ldcs(reinterpret_cast<const float4 *>(f.x + oprev));
+            T4 = __ldcs(reinterpret_cast<const float4 *>(f.T + oprev));
+            h4 = __ldcs(reinterpret_cast<const float4 *>(f.nH + oprev));
+#else
             x4 = *reinterpret_cast<const float4 *>(f.x + oprev);
             T4 = *reinterpret_cast<const float4 *>(f.T + oprev);
             h4 = __ldg(reinterpret_cast<const float4 *>(f.nH + oprev));
+#endif
             srcw = __ldg(f.src_bits + ((unsigned)oprev >> 5));
         }
         // ---- closure of the staged quad
@@ -291,7 +315,11 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
                 nib |= chem_fast2<FLAGS>(pend.v[p][0], pend.v[p][1], pend.v[p][2], pend.v[p][3], xs[p], Ts[p], hs[p], c,
                                          (srcn >> (2 * p)) & 3u)
                        << (2 * p);
+#if ATON_V4_CS & 2       // written once, not read again this step: streaming stores
+#define ATON_ST4(ptr, A, B) __stcs(reinterpret_cast<float4 *>(ptr + oprev), make_float4(lo(A), hi(A), lo(B), hi(B)))
+#else
 #define ATON_ST4(ptr, A, B) *reinterpret_cast<float4 *>(ptr + oprev) = make_float4(lo(A), hi(A), lo(B), hi(B))
+#endif
             ATON_ST4(f.N1, pend.v[0][0], pend.v[1][0]);
             ATON_ST4(f.Gx1, pend.v[0][1], pend.v[1][1]);
             ATON_ST4(f.Gy1, pend.v[0][2], pend.v[1][2]);
