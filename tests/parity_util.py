@@ -58,9 +58,11 @@ def max_rel_errors(g, st, c):
 def l1_errors(g, st, c):
     """BASELINE.json full-run metric: relative L1 error per field (F measured against c*N)."""
     err = {}
-    err["N"] = float(np.abs(g["N"] - st.N).sum() / np.abs(st.N).sum())
+    nsum = float(np.abs(st.N).sum())
+    rel = lambda num: float(num / nsum) if nsum > 0 else (0.0 if num == 0 else float("inf"))   # dark region: exact zeros
+    err["N"] = rel(np.abs(g["N"] - st.N).sum())
     dF = np.abs(g["Fx"] - st.Fx) + np.abs(g["Fy"] - st.Fy) + np.abs(g["Fz"] - st.Fz)
-    err["F"] = float(dF.sum() / (c * np.abs(st.N).sum()))
+    err["F"] = rel(dF.sum() / c)
     err["x"] = float(np.abs(g["x"] - st.x).sum() / np.abs(st.x).sum())
     err["T"] = float(np.abs(g["T"] - st.T).sum() / np.abs(st.T).sum())
     err["x_vol"] = float(abs(g["x"].astype(np.float64).mean() - st.x.mean()))
