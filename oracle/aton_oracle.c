@@ -20,8 +20,9 @@
  * matrix (P4), photon budget + brute-force root of the backward-Euler system (P5), equilibrium
  * closed form (P6), Stroemgren volume (P7), first step from vacuum (P8), cube symmetry (P9),
  * textbook spot values of the rate fits (S7).
- * PARITY UNPINNED: the absolute values of the cooling-rate fits (orc_rates: zeta_*) beyond
- * order-of-magnitude textbook values, and hence the T evolution away from the thermal fixed point.
+ * PARITY UNPINNED: the absolute values of the collisional cooling fits (orc_rates: z_exc, z_ci) beyond
+ * order-of-magnitude textbook values (z_rec is pinned to the textbook k T beta table, z_ff to its prefactor),
+ * and hence the T evolution of collisionally cooled gas away from the thermal fixed point.
  */
 #include <math.h>
 #include <stdlib.h>

@@ -37,6 +37,23 @@ def test_recombination_fits_match_textbook_table(orc):
     assert orc.rates(1e4)["alpha_B"] == pytest.approx(2.59e-13, rel=2e-3)
 
 
+def test_recombination_cooling_fits_match_textbook_table(orc):
+    """zeta_rec = k T beta with the textbook beta_A, beta_B: pins the absolute value of the recombination-cooling
+    fits (the largest cooling term of photo-ionised gas at 1e4 K) to 5 %."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "osterbrock_recombination_cooling.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for T, bA, bB in rows:
+        T, bA, bB = float(T), float(bA), float(bB)
+        r = orc.rates(T)
+        assert r["z_recA"] == pytest.approx(KB * T * bA, rel=0.05)
+        assert r["z_recB"] == pytest.approx(KB * T * bB, rel=0.05)
+    # bremsstrahlung: the textbook 1.42e-27 g_ff sqrt(T) with a Gaunt factor between 1.1 and 1.5
+    for T in (1e4, 1e6):
+        g = orc.rates(T)["z_ff"] / (1.42e-27 * math.sqrt(T))
+        assert 1.1 <= g <= 1.5
+
+
 def test_collisional_and_cooling_fits_orders_of_magnitude(orc):
     """Independent (different-author) closed forms: Voronov (1997) for the collisional ionisation
     rate (within 25 %), Cen (1992) for the cooling rates (within a factor 2) over 1e4-1e6 K;
