@@ -19,10 +19,11 @@
  * binomial (P1), vacuum conservation (P2), realizability (P3), diffusion-limit amplification
  * matrix (P4), photon budget + brute-force root of the backward-Euler system (P5), equilibrium
  * closed form (P6), Stroemgren volume (P7), first step from vacuum (P8), cube symmetry (P9),
- * textbook spot values of the rate fits (S7).
- * PARITY UNPINNED: the absolute values of the collisional cooling fits (orc_rates: z_exc, z_ci) beyond
- * order-of-magnitude textbook values (z_rec is pinned to the textbook k T beta table, z_ff to its prefactor),
- * and hence the T evolution of collisionally cooled gas away from the thermal fixed point.
+ * textbook spot values of the rate fits (S7): alpha_A/B (3 %), z_rec (5 %), z_ff prefactor, z_exc against the
+ * two-level Lyman-alpha rate (factor 2) and its Boltzmann temperature (1e-3), the Compton coefficient from CODATA
+ * constants (1 %) and its sign, the 10 % rule as an inequality on every accepted sub-step, F' = c n N' on f = 1 beams.
+ * LOOSEST PIN: the collisional-ionisation fit beta (and z_ci = 13.6 eV * beta) is held to 25 % of an independent
+ * (different-author) closed form only; no table value is in the container to do better.
  */
 #include <math.h>
 #include <stdlib.h>
@@ -302,9 +303,11 @@ static double edot_est(double N, double x, double T, double nH, const orc_params
     return H - Lam;
 }
 
-/* O4 full per-cell operator Phi of Eq.A4 (L435-437): sub-cycled over the transport step dt. */
-int orc_chem_cell(double *N, double F[3], double *x, double *T, double nH, double dt,
-                  const orc_params *p) {
+/* O4 full per-cell operator Phi of Eq.A4 (L435-437): sub-cycled over the transport step dt.
+ * `trace` (may be NULL) receives, for the first `trace_cap` sub-steps, the 4 numbers (dts, N, x, T) at the START of
+ * each sub-step: the pin of the 10 % rule reads them; nothing is computed from them. */
+int orc_chem_cell_trace(double *N, double F[3], double *x, double *T, double nH, double dt,
+                        const orc_params *p, double *trace, int trace_cap) {
     double t_left = dt;
     int nsub = 0;
     while (t_left > 0.0 && nsub < p->max_sub) {
@@ -314,11 +317,28 @@ int orc_chem_cell(double *N, double F[3], double *x, double *T, double nH, doubl
             double Ed = fabs(edot_est(*N, *x, *T, nH, p));
             if (Ed * t_left > p->eps_sub * E) dts = p->eps_sub * E / Ed;
         }
+        if (trace && nsub < trace_cap) {
+            trace[4 * nsub + 0] = dts; trace[4 * nsub + 1] = *N; trace[4 * nsub + 2] = *x; trace[4 * nsub + 3] = *T;
+        }
         orc_chem_substep(N, F, x, T, nH, dts, p);
         t_left -= dts;
         nsub++;
     }
     return nsub;
+}
+
+int orc_chem_cell(double *N, double F[3], double *x, double *T, double nH, double dt,
+                  const orc_params *p) {
+    return orc_chem_cell_trace(N, F, x, T, nH, dt, p, NULL, 0);
+}
+
+/* Read-only views for the pins: out[0] = Lambda, out[1] = dLambda/dlnT of cooling_fn, out[2] = the net heating rate
+ * H - Lambda that picks the sub-step (edot_est), all at (N, x, T, nH). */
+void orc_cooling_probe(double N, double x, double T, double nH, const orc_params *p, double out[3]) {
+    orc_rates_t r;
+    orc_rates(T, &r);
+    cooling_fn(x, T, nH, orc_clumping(nH, p), &r, p, &out[0], &out[1]);
+    out[2] = edot_est(N, x, T, nH, p);
 }
 
 /* chemistry over the whole grid; returns total sub-cycles, *sub_max = largest per-cell count */

@@ -65,6 +65,9 @@ def lib():
         L.orc_chem_substep.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, C.POINTER(Params)]
         L.orc_chem_cell.restype = C.c_int
         L.orc_chem_cell.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, C.POINTER(Params)]
+        L.orc_chem_cell_trace.restype = C.c_int
+        L.orc_chem_cell_trace.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, C.POINTER(Params), _dp, C.c_int]
+        L.orc_cooling_probe.argtypes = [C.c_double] * 4 + [C.POINTER(Params), _dp]
         L.orc_chemistry.restype = C.c_longlong
         L.orc_chemistry.argtypes = [C.c_long] + [_dp] * 7 + [C.c_double, C.POINTER(Params),
                                                              C.POINTER(C.c_longlong)]
@@ -160,6 +163,22 @@ def chem_cell(N: float, F, x: float, T: float, nH: float, dt: float, p: Params):
     Fa = np.array(F, dtype=np.float64)
     ns = lib().orc_chem_cell(C.byref(n_), _p(Fa), C.byref(x_), C.byref(t_), nH, dt, C.byref(p))
     return n_.value, Fa, x_.value, t_.value, int(ns)
+
+
+def chem_cell_trace(N: float, F, x: float, T: float, nH: float, dt: float, p: Params, cap: int = 4096):
+    """chem_cell plus the (dts, N, x, T) at the start of every sub-step: returns (N', F', x', T', n_sub, trace[n,4])."""
+    n_, x_, t_ = C.c_double(N), C.c_double(x), C.c_double(T)
+    Fa = np.array(F, dtype=np.float64)
+    tr = np.zeros((cap, 4))
+    ns = lib().orc_chem_cell_trace(C.byref(n_), _p(Fa), C.byref(x_), C.byref(t_), nH, dt, C.byref(p), _p(tr), cap)
+    return n_.value, Fa, x_.value, t_.value, int(ns), tr[:min(ns, cap)]
+
+
+def cooling_probe(N: float, x: float, T: float, nH: float, p: Params) -> Dict[str, float]:
+    """Lambda [erg cm^-3 s^-1], dLambda/dlnT and the net heating rate H - Lambda of the sub-step rule."""
+    out = np.zeros(3)
+    lib().orc_cooling_probe(float(N), float(x), float(T), float(nH), C.byref(p), _p(out))
+    return {"Lambda": out[0], "Lambda_T": out[1], "edot": out[2]}
 
 
 class State:

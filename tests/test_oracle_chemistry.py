@@ -301,3 +301,121 @@ def test_subcycled_result_converges_with_tolerance(orc):
     e = [abs(r[3] - Tref) for r in res[:3]]
     assert e[0] > e[1] > e[2]
     assert e[1] / e[2] == pytest.approx(2.0, rel=0.35)
+
+
+# ------------------------------------------------------------------ collisional excitation, Compton, the 10 % rule
+def _gold(name):
+    out = {}
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+def test_collisional_excitation_is_the_lyman_alpha_two_level_rate(orc):
+    """z_exc (Cen 1992 fit, reading S7) against first principles: (i) its Boltzmann temperature, read off the ratio of
+    two temperatures, is the Lyman-alpha excitation energy h c / (lambda k) to 1e-3; (ii) its size at 1e4 and 2e4 K is
+    the two-level rate q12 h nu = 8.629e-6 Omega12/(g1 sqrt T) exp(-E12/kT) h nu with the textbook 1s-2p collision
+    strength, within a factor 2 at 1e4 K and 3 at 2e4 K (the fit also carries the higher levels and the rise of Omega
+    with T, so it must not fall BELOW the 1s-2p rate taken with the 1e4 K collision strength)."""
+    g = _gold("collisional_excitation_and_compton.txt")
+    hnu = g["h_planck_erg_s"] * g["c_cm_s"] / (g["lyman_alpha_A"] * 1e-8)
+    T12 = hnu / g["k_boltz_erg_K"]
+    assert T12 == pytest.approx(118352.0, rel=1e-4)                     # 10.2 eV
+    T1, T2 = 1.0e4, 2.0e4
+    z1, z2 = orc.rates(T1)["z_exc"], orc.rates(T2)["z_exc"]
+    # z = K exp(-T12/T) / (1 + sqrt(T/1e5)): undo the slowly varying denominator, solve the ratio for T12
+    boltz = math.log(z2 * (1 + math.sqrt(T2 / 1e5)) / (z1 * (1 + math.sqrt(T1 / 1e5)))) / (1 / T1 - 1 / T2)
+    assert boltz == pytest.approx(T12, rel=1e-3)
+    for T, z in ((T1, z1), (T2, z2)):
+        lo, hi = [g["rate_prefactor"] * om / (g["g_ground"] * math.sqrt(T)) * math.exp(-T12 / T) * hnu
+                  for om in (g["omega_1s2p_lo"], g["omega_1s2p_hi"])]
+        assert lo <= z <= (2.0 if T == T1 else 3.0) * hi, (T, z, lo, hi)
+    # the logarithmic derivative used by the implicit energy update carries the same Boltzmann temperature
+    assert orc.rates(T1)["dl_exc"] == pytest.approx(T12 / T1, rel=0.02)
+
+
+def test_compton_cooling_coefficient_and_sign(orc):
+    """Compton term of the cooling function (reading S7): Lambda_C = 4 sigma_T a_rad T_cmb^4 k_B (T - T_cmb) n_e/(m_e c)
+    with T_cmb = 2.726 (1+z): the coefficient to 1 % from CODATA constants, the (1+z)^4 scaling, the sign change at
+    T_cmb, the linearity in n_e = x n_H, and `redshift < 0` switching it off."""
+    g = _gold("collisional_excitation_and_compton.txt")
+    k0 = 4 * g["sigma_thomson_cm2"] * g["a_rad_erg_cm3_K4"] * g["k_boltz_erg_K"] * g["T_cmb_K"] ** 4 / (g["m_electron_g"] * g["c_cm_s"])
+    assert k0 == pytest.approx(5.62e-36, rel=2e-3)
+    nH = 2.0e-4
+    off = _params(orc, redshift=-1.0)
+    for z in (0.0, 7.0, 9.0):
+        on = _params(orc, redshift=z)
+        tcmb = g["T_cmb_K"] * (1 + z)
+        for x in (0.3, 1.0):
+            for T in (1.0e4, 300.0, 0.5 * tcmb):
+                lam_c = orc.cooling_probe(0.0, x, T, nH, on)["Lambda"] - orc.cooling_probe(0.0, x, T, nH, off)["Lambda"]
+                want = k0 * (1 + z) ** 4 * (x * nH) * (T - tcmb)
+                assert lam_c == pytest.approx(want, rel=1e-2)
+                assert (lam_c > 0) == (T > tcmb)                 # cools above the CMB temperature, heats below
+                # its d/dlnT is k T (the implicit energy update's denominator)
+                dl = orc.cooling_probe(0.0, x, T, nH, on)["Lambda_T"] - orc.cooling_probe(0.0, x, T, nH, off)["Lambda_T"]
+                assert dl == pytest.approx(k0 * (1 + z) ** 4 * x * nH * T, rel=1e-2)
+        # gas exactly at the CMB temperature neither gains nor loses through it
+        assert orc.cooling_probe(0.0, 0.5, tcmb, nH, on)["Lambda"] == pytest.approx(
+            orc.cooling_probe(0.0, 0.5, tcmb, nH, off)["Lambda"], rel=1e-12)
+    # the sub-step sees it: hot ionised gas with no photons cools faster with the CMB at z = 9 than without
+    a = orc.chem_substep(0.0, [0, 0, 0], 1.0, 2.0e4, nH, 1e12, _params(orc, redshift=9.0, coll_ion=0))
+    b = orc.chem_substep(0.0, [0, 0, 0], 1.0, 2.0e4, nH, 1e12, _params(orc, redshift=-1.0, coll_ion=0))
+    assert a[2] == b[2] and a[3] < b[3]
+    dE = 1.5 * KB * nH * (1 + a[2]) * (b[3] - a[3])               # energy the CMB took in 1e12 s
+    assert dE == pytest.approx(1e12 * k0 * 1e4 * a[2] * nH * (2.0e4 - 27.26), rel=0.02)
+
+
+def test_heating_estimate_is_absorbed_energy_minus_cooling(orc):
+    """The rate that picks the sub-step (steps 2-3 of reading S5): H - Lambda with H = n_H (1-x) c N (e sigma_e - e0 sigma_n),
+    i.e. the photo-heating of the photons absorbed per second; H alone where nothing cools (cold, neutral)."""
+    p = _params(orc, redshift=-1.0)
+    nH, x, T, N = 1e-3, 1e-6, 50.0, 1e-8
+    pr = orc.cooling_probe(N, x, T, nH, p)
+    H = nH * (1 - x) * C * N * (p.e_photon_eV * p.sigma_e - 13.6 * p.sigma_n) * EV
+    assert pr["Lambda"] < 1e-12 * H
+    assert pr["edot"] == pytest.approx(H, rel=1e-9)
+    # with C_I the absorption (and so the heating) is C_I times faster
+    q = _params(orc, redshift=-1.0, clump_i_a=50.0, clump_i_b=0.2)
+    assert orc.cooling_probe(N, x, T, nH, q)["edot"] == pytest.approx(H * 50.0 * nH ** 0.2, rel=1e-9)
+    # no photons: the estimate is minus the cooling function
+    hot = orc.cooling_probe(0.0, 0.9, 3e4, nH, p)
+    assert hot["edot"] == pytest.approx(-hot["Lambda"], rel=1e-14) and hot["Lambda"] > 0
+
+
+@pytest.mark.parametrize("kw", [dict(N=1e-2, x=1.2e-3, T=100.0, nH=1e-3, dt=5.6e9),            # config 1 source cell
+                                dict(N=3e-4, x=0.01, T=300.0, nH=1e-3, dt=2e10),
+                                dict(N=0.0, x=0.999, T=8.0e5, nH=0.3, dt=4e11),                  # pure cooling
+                                dict(N=5e-3, x=0.5, T=2.0e4, nH=1.0, dt=2e11, clump_model=1, recomb_case=0, nH_mean=1e-4),
+                                dict(N=1e-9, x=1e-3, T=100.0, nH=1e-4, dt=1e10)])               # quiet cell: one sub-step
+def test_ten_percent_rule_holds_on_every_substep(orc, kw):
+    """Reading S5 step 3 (the Anninos 10 % rule), as an exact statement on the accepted sub-steps: each has
+    |H - Lambda| dts <= eps E at its START state; it is the LARGEST such step (dts = t_left, or equality);
+    the sub-steps add up to dt; the state handed to the next sub-step is the previous sub-step's result."""
+    kw = dict(kw)
+    N, x, T, nH, dt = (kw.pop(k) for k in ("N", "x", "T", "nH", "dt"))
+    eps = 0.1
+    p = _params(orc, cooling=1, coll_ion=1, redshift=8.0, eps_sub=eps, **kw)
+    Nn, _, xn, Tn, ns, tr = orc.chem_cell_trace(N, [0, 0, 0], x, T, nH, dt, p)
+    assert ns == len(tr) and ns >= 1
+    assert tr[:, 0].sum() == pytest.approx(dt, rel=1e-12)
+    assert (tr[0, 1], tr[0, 2], tr[0, 3]) == (N, x, T)
+    t_left = dt
+    for k in range(ns):
+        dts, Nk, xk, Tk = tr[k]
+        E = 1.5 * KB * nH * (1 + xk) * Tk
+        ed = abs(orc.cooling_probe(Nk, xk, Tk, nH, p)["edot"])
+        assert ed * dts <= eps * E * (1 + 1e-12)
+        if k < ns - 1:
+            assert ed * dts == pytest.approx(eps * E, rel=1e-12)          # limited by the rule, not by t_left
+        else:
+            assert dts == pytest.approx(t_left, rel=1e-9, abs=1e-6 * dt)  # the last one takes what is left
+        # the next sub-step starts where this one ended
+        nxt = orc.chem_substep(Nk, [0, 0, 0], xk, Tk, nH, dts, p)
+        got = (tr[k + 1, 1], tr[k + 1, 2], tr[k + 1, 3]) if k < ns - 1 else (Nn, xn, Tn)
+        assert got == (nxt[0], nxt[2], nxt[3])
+        t_left -= dts
+    if kw == {}:
+        assert (ns > 5) == (N >= 3e-4)

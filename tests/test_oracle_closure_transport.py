@@ -141,12 +141,26 @@ def test_oblique_beam_one_step(orc):
     nd = np.array([1.0, 1.0, 0.0]) / math.sqrt(2)
     F = [C * N * nd[a] for a in range(3)]
     dx = 3.0e21; dt = mu * dx / C
-    N1, *_ = orc.transport(N, F[0], F[1], F[2], C, dx, dt)
+    N1, Fx1, Fy1, Fz1 = orc.transport(N, F[0], F[1], F[2], C, dx, dt)
     want = (1 - 2 * mu) * prof
     for ax, d in ((1, 0), (0, 1)):                                       # array axis, direction
         want = want + 0.5 * mu * (1 - nd[d]) * np.roll(prof, -1, axis=ax) \
                     + 0.5 * mu * (1 + nd[d]) * np.roll(prof, +1, axis=ax)
     assert np.allclose(N1[4], want, rtol=1e-13)
+    # f = 1 data: P = n(x)n N, so every flux row of F is c n_j times the flux row of N and the scheme gives
+    # F' = c n N' exactly -- this is where the OFF-DIAGONAL pressure P_xy enters (a dropped or transposed P_xy fails)
+    assert np.allclose(Fx1, C * nd[0] * N1, rtol=1e-13) and np.allclose(Fy1, C * nd[1] * N1, rtol=1e-13)
+    assert np.abs(Fz1).max() <= 1e-13 * C * N1.max()
+    # a generic direction with all three components and all six off-diagonal terms live
+    nd = np.array([2.0, -3.0, 6.0]) / 7.0
+    N = rng.uniform(0.5, 1.5, size=(n, n, n))
+    N1, Fx1, Fy1, Fz1 = orc.transport(N, C * N * nd[0], C * N * nd[1], C * N * nd[2], C, dx, dt)
+    want = (1 - 3 * mu) * N
+    for ax, d in ((2, 0), (1, 1), (0, 2)):
+        want = want + 0.5 * mu * (1 - nd[d]) * np.roll(N, -1, axis=ax) + 0.5 * mu * (1 + nd[d]) * np.roll(N, +1, axis=ax)
+    assert np.allclose(N1, want, rtol=1e-13)
+    for Fj, nj in ((Fx1, nd[0]), (Fy1, nd[1]), (Fz1, nd[2])):
+        assert np.allclose(Fj, C * nj * N1, rtol=1e-12)
 
 
 def _random_realizable(n, rng, fmax=0.99):
