@@ -77,10 +77,12 @@ typedef struct {
     long long n_nonfinite;        /* cells holding a NaN/Inf in any of N, F, x, T */
     long long subcycles_total;    /* chemistry sub-cycles summed over cells and steps since aton_set_fields */
     long long subcycles_max;      /* largest per-cell, per-step sub-cycle count seen */
-    long long cells_subcycled;    /* cell-steps handed to the fix-up kernel: cells that needed more than one
-                                     sub-cycle (variants 2-4) and, for variant 4, the source cells */
+    long long cells_subcycled;    /* cell-steps redone outside the one-sub-step fast path: cells that needed more than
+                                     one sub-cycle (variants 2, 4) and, for variant 4, the source cells */
     long long steps_done;         /* steps since aton_set_fields */
     double time_s;                /* sum of dt since aton_set_fields */
+    long long cells_fp64;         /* of cells_subcycled: cell-steps whose sub-cycling was redone in fp64 because heating
+                                     and cooling cancelled (the 10 % rule's sub-step is then ill-conditioned in fp32) */
 } aton_diag_t;
 
 /* Create a context: allocates 11 float32 device arrays of nx*ny*nz (7 fields + 4 ping-pong) and one bit
@@ -117,15 +119,14 @@ int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float 
 /* Global diagnostics of the current state (deterministic two-pass reduction).  Synchronises. */
 int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
-/* Select the step kernel: 0 = reference kernel (one thread per cell, neighbours from global
- * memory); 1 = tiled streaming kernel; 2 = fused packed-arithmetic kernel + sub-cycle fix-up kernel;
- * 3 = variant 2's arithmetic with full CTA tiles and a split-phase barrier (nx % 128 == 0, ny % tile_y == 0);
- * 4 (default) = warp-autonomous tiles, no inter-warp synchronisation, sources injected by the fix-up
- * kernel (nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0 and ny % 2 == 0).  A grid a variant cannot tile runs the
- * variant-2 kernel.
- * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 8, 14} rows, default 6;
- * variant 3: tile_y in {4, 8, 16}, default 8; variant 4: tile_y 4 = 32 x 4 warp tiles (default), 2 = 64 x 2; tile_z = planes per z-chunk);
- * results agree between variants to rounding and do not depend on the tile shape.  ATON_EINVAL otherwise. */
+/* Select the step kernel: 4 (default, the product) = warp-autonomous tiles, no inter-warp synchronisation; source
+ * cells and cells that need sub-cycling are redone by the producing warp in batches of 32, stiff cells in fp64
+ * (needs nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0 and ny % 2 == 0; any other grid runs the variant-2 kernel);
+ * 2 = CTA-tiled fused kernel + mask-scanning fix-up kernel (the fallback for grids variant 4 cannot tile);
+ * 0 = reference kernel (one thread per cell, neighbours from global memory; a cross-check).
+ * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 14} rows; variant 4: tile_y 4 = 32 x 4
+ * warp tiles (default), 2 = 64 x 2; tile_z = planes per z-chunk); results agree between variants to rounding and do
+ * not depend on the tile shape (bitwise).  ATON_EINVAL for anything else (variants 1 and 3 of round 1 are gone). */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */
@@ -138,6 +139,10 @@ int aton_set_timing(aton_t *ctx, int on);
 
 /* Sum [ms] and number of the bracketed launches since aton_set_timing(ctx, 1).  Synchronises. */
 int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches);
+
+/* The same for the second kernel of a step (variant 4: the fp64 redo of stiff cells; variant 2: the fix-up kernel).
+ * Variant 4 redoes its sub-cycling cells inside the step kernel, so their cost is part of aton_kernel_time. */
+int aton_fixup_time(aton_t *ctx, double *ms_total, long long *n_launches);
 
 /* ---- slab decomposition along z (the paper's multi-GPU mode, PAPER.md:L471-484,
  * re-cut as z slabs whose one-plane halo of (N, F) is one contiguous block per field) ----

@@ -19,7 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt", "aton_step",
            "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_set_timing",
-           "aton_kernel_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
+           "aton_kernel_time", "aton_fixup_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
            "aton_reduce_sums", "aton_free", "aton_last_error")
 NSUMS = 14
 
@@ -46,7 +46,7 @@ class Diag(C.Structure):
                 ("f_max", C.c_double), ("N_min", C.c_double), ("frac_x_half", C.c_double),
                 ("n_nonfinite", C.c_longlong), ("subcycles_total", C.c_longlong),
                 ("subcycles_max", C.c_longlong), ("cells_subcycled", C.c_longlong),
-                ("steps_done", C.c_longlong), ("time_s", C.c_double)]
+                ("steps_done", C.c_longlong), ("time_s", C.c_double), ("cells_fp64", C.c_longlong)]
 
 
 class AtonError(RuntimeError):
@@ -91,6 +91,8 @@ def load_library(path: Optional[str] = None):
     L.aton_set_timing.argtypes = [vp, C.c_int]
     L.aton_kernel_time.restype = C.c_int
     L.aton_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.aton_fixup_time.restype = C.c_int
+    L.aton_fixup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.aton_init_slab.restype = C.c_int
     L.aton_init_slab.argtypes = [C.POINTER(vp), C.POINTER(Grid), C.POINTER(Box), C.POINTER(Params), vp, C.c_int, C.c_int]
     L.aton_halo_pack.restype = C.c_int
@@ -231,6 +233,12 @@ class Aton:
         """(sum of ms, launches) of the event-bracketed dominant step kernel since set_timing(True)."""
         ms, n = C.c_double(), C.c_longlong()
         self._check(self._L.aton_kernel_time(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
+
+    def fixup_time(self):
+        """(sum of ms, launches) of the event-bracketed second kernel of a step since set_timing(True)."""
+        ms, n = C.c_double(), C.c_longlong()
+        self._check(self._L.aton_fixup_time(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
 
     def launch_count(self) -> int:

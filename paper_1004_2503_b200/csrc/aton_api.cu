@@ -1,6 +1,7 @@
 // C ABI of the ATON hot path (include/aton.h): context, uploads/downloads, source lists, the step
 // loop and the diagnostics.  The host only drives; every step of the path runs in
-// the kernels of aton_step_tiled.cuh / aton_step_ref.cuh / aton_reduce.cuh.
+// the kernels of aton_step_v4.cuh (product), aton_fixup.cuh, aton_step_fused.cuh / aton_step_ref.cuh
+// (fallback / cross-check) and aton_reduce.cuh.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -16,9 +17,8 @@
 #include "aton_physics.cuh"
 #include "aton_reduce.cuh"
 #include "aton_step_ref.cuh"
-#include "aton_step_tiled.cuh"
 #include "aton_step_fused.cuh"
-#include "aton_step_v3.cuh"
+#include "aton_fixup.cuh"
 #include "aton_step_v4.cuh"
 
 using namespace aton;
@@ -27,6 +27,7 @@ namespace {
 
 constexpr double K_BOLTZ = 1.380649e-16, EV_ERG = 1.602176634e-12, E0_EV = 13.6;
 constexpr int REDUCE_BLOCKS = 148 * 8;
+constexpr int N_STATS = 4;
 
 char g_init_error[512] = "";
 
@@ -48,10 +49,18 @@ struct aton_ctx {
     unsigned *src_mask = nullptr;
     int *src_cell = nullptr;
     float *src_rho = nullptr;
+    double *src_rho_d = nullptr;
     int n_src = 0;
-    unsigned long long *stats = nullptr;   // device [3]
-    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variants 2-4)
+    int device = 0;                        // the device current at aton_init; every entry point runs there
+    unsigned long long *stats = nullptr;   // device [4]
+    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variant 2)
     unsigned *src_bits = nullptr;          // device, 1 bit per cell: the cell holds a source (variant 4)
+    int *stiff_q = nullptr;                // device [stiff_cap]: ids of the cells to redo in fp64 (variant 4)
+    unsigned *stiff_n = nullptr;           // device [2]
+    unsigned stiff_cap = 0;
+    FixArgs *fixargs = nullptr;            // device [2]: what the cold paths of variant 4 read, per ping-pong parity
+    bool fix_dirty = true;                 // fixargs must be rewritten (dt, sources, <n_H> or buffers changed)
+    double fix_dt = -1.0;
     long long fast_subcycles = 0;          // variant 2: one sub-cycle per cell and step, counted on the host
     double *partials = nullptr;            // device [REDUCE_BLOCKS+1][R_COUNT]
     double nH_mean = 1.0;
@@ -59,8 +68,9 @@ struct aton_ctx {
     long long steps_done = 0, launches = 0;
     double time_s = 0;
     int variant = 4, tile_y = 0, tile_z = 0;
-    bool timing = false;                   // aton_set_timing: CUDA events around the dominant step kernel
-    std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch
+    bool timing = false;                   // aton_set_timing: CUDA events around the kernels of a step
+    std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch of the dominant step kernel
+    std::vector<cudaEvent_t> ev_fix;       // the same for the second kernel of a step (fp64 redo / mask fix-up)
     char err[512] = "";
 };
 
@@ -122,19 +132,64 @@ StepConst make_step_const(const aton_ctx *ctx, double dt) {
     return s;
 }
 
-FieldsIO make_io(const aton_ctx *ctx) {
+StepConstD make_step_const_d(const aton_ctx *ctx, double dt) {
+    const aton_params_t &p = ctx->p;
+    const double kb15 = 1.5 * K_BOLTZ;
+    StepConstD s{};
+    s.dt = dt;
+    s.cs = ctx->c * p.sigma_n;
+    s.heat_K = (p.e_photon_eV * p.sigma_e / p.sigma_n - E0_EV) * EV_ERG / kb15;
+    s.heat_rate_K = ctx->c * (p.e_photon_eV * p.sigma_e - E0_EV * p.sigma_n) * EV_ERG / kb15;
+    s.zrec0 = (p.recomb_case == 0 ? 1.778e-29 : 3.435e-30) / kb15;
+    s.zff0 = 1.42e-27 / kb15;
+    s.zexc0 = 7.5e-19 / kb15;
+    s.zci_over_beta = E0_EV * EV_ERG / kb15;
+    const double zp1 = 1.0 + p.redshift;
+    s.compton0 = p.redshift >= 0.0 ? 5.65e-36 * zp1 * zp1 * zp1 * zp1 / kb15 : 0.0;
+    s.t_cmb = 2.726 * zp1;
+    s.eps_sub = p.eps_sub;
+    s.max_sub = p.max_sub;
+    s.clump_model = p.clump_model;
+    if (p.clump_model == 1) {
+        s.clump_k0 = p.clump_a - p.clump_b;
+        s.clump_k1 = p.clump_b / ctx->nH_mean;
+    } else {
+        s.clump_k0 = p.clump_a;
+        s.clump_k1 = p.clump_b;
+    }
+    s.ci_k0 = p.clump_i_a > 0.0 ? p.clump_i_a : 0.0;
+    s.ci_k1 = p.clump_i_b;
+    return s;
+}
+
+FieldsIO make_io(const aton_ctx *ctx, int cur) {
     FieldsIO f{};
-    const int a = ctx->cur, b = 1 - ctx->cur;
+    const int a = cur, b = 1 - cur;
     f.N = ctx->rad[a][0]; f.Gx = ctx->rad[a][1]; f.Gy = ctx->rad[a][2]; f.Gz = ctx->rad[a][3];
     f.N1 = ctx->rad[b][0]; f.Gx1 = ctx->rad[b][1]; f.Gy1 = ctx->rad[b][2]; f.Gz1 = ctx->rad[b][3];
     f.x = ctx->x; f.T = ctx->T; f.nH = ctx->nH;
-    f.src_mask = ctx->src_mask; f.src_cell = ctx->src_cell; f.src_rho = ctx->src_rho;
+    f.src_mask = ctx->src_mask; f.src_cell = ctx->src_cell; f.src_rho = ctx->src_rho; f.src_rho_d = ctx->src_rho_d;
     f.n_src = ctx->n_src;
     f.stats = ctx->stats;
     f.defer_mask = ctx->defer_mask;
     f.src_bits = ctx->src_bits;
-    f.fix_inject = 0;
+    f.stiff_q = ctx->stiff_q; f.stiff_n = ctx->stiff_n; f.stiff_cap = ctx->stiff_cap;
     return f;
+}
+
+__global__ void write_fixargs_kernel(FixArgs a0, FixArgs a1, FixArgs *dst) { dst[0] = a0; dst[1] = a1; }
+
+// variant 4's cold paths (v4_fix_batch, step_stiff_kernel) read their arguments from global memory; rewrite them
+// (stream-ordered, no host synchronisation) only when something they hold has changed
+cudaError_t sync_fixargs(aton_ctx *ctx, const StepConst &sc, const StepConstD &scd, double dt) {
+    if (!ctx->fix_dirty && ctx->fix_dt == dt) return cudaSuccess;
+    FixArgs a[2];
+    for (int cur = 0; cur < 2; cur++) { a[cur].f = make_io(ctx, cur); a[cur].c = sc; a[cur].cd = scd; }
+    write_fixargs_kernel<<<1, 1, 0, ctx->stream>>>(a[0], a[1], ctx->fixargs);
+    ctx->launches++;
+    ctx->fix_dirty = false;
+    ctx->fix_dt = dt;
+    return cudaGetLastError();
 }
 
 // aton_set_timing: an event right before / after the dominant kernel of a step
@@ -146,57 +201,67 @@ void time_mark(aton_ctx *ctx) {
     ctx->ev.push_back(e);
 }
 
+void fix_mark(aton_ctx *ctx) {
+    if (!ctx->timing) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, ctx->stream);
+    ctx->ev_fix.push_back(e);
+}
+
 template <int FLAGS>
-cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc) {
+cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc, const StepConstD &scd) {
     if (ctx->variant == 0) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
         time_mark(ctx);
-        step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc);
+        step_ref_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc, scd);
         time_mark(ctx);
         return cudaGetLastError();
     }
-    if (ctx->variant == 1) {
+    // variant 4 needs nx % 32 == 0 and ny % 4 == 0 (or nx % 64 == 0 and ny % 2 == 0); other grids run the variant-2
+    // kernel.  Variant 4 leaves the source cells and the sub-cycling cells to its own warp-level redo + the fp64
+    // kernel; variant 2 injects in the step kernel and flags the sub-cycling cells for step_fixup_kernel.
+    const int wxq4 = ctx->variant == 4 ? v4_pick_wxq(ctx->g, ctx->tile_y) : 0;
+    if (ctx->slab && !wxq4) return cudaErrorNotSupported;    // checked with a message in aton_step
+    ctx->fast_subcycles += (long long)ctx->ncell;
+    cudaError_t e;
+    if (wxq4) {
         time_mark(ctx);
-        const cudaError_t e = launch_step_tiled<FLAGS>(f, ctx->g, sc, ctx->tile_y, ctx->tile_z, ctx->stream);
+        e = launch_step_v4<FLAGS>(f, ctx->g, sc, ctx->fixargs + ctx->cur, wxq4, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
+                                  ctx->slab ? ctx->nz_local + 1 : ctx->g.nz);
         time_mark(ctx);
+        if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;   // without cooling nothing sub-cycles: no cell can be stiff
+        ctx->launches++;
+        fix_mark(ctx);
+        e = launch_step_stiff<FLAGS>(ctx->fixargs + ctx->cur, ctx->stream);
+        fix_mark(ctx);
         return e;
     }
-    // variant 4 needs nx % 32 == 0, ny % 4 == 0; variant 3 nx % 128 == 0, ny % TY == 0; other grids run the
-    // variant-2 kernel.  Only variant 4 leaves the source injection to the fix-up kernel.
-    const int wxq4 = ctx->variant == 4 ? v4_pick_wxq(ctx->g, ctx->tile_y) : 0;
-    const bool use4 = wxq4 != 0;
-    if (ctx->slab && !use4) return cudaErrorNotSupported;    // checked with a message in aton_step
-    const int ty3 = ctx->variant == 3 ? v3_pick_ty(ctx->g, ctx->tile_y) : 0;
-    FieldsIO f2 = f;
-    f2.fix_inject = use4 ? 1 : 0;
     time_mark(ctx);
-    cudaError_t e = use4 ? launch_step_v4<FLAGS>(f2, ctx->g, sc, wxq4, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
-                                                 ctx->slab ? ctx->nz_local + 1 : ctx->g.nz)
-                    : ty3 ? launch_step_v3<FLAGS>(f2, ctx->g, sc, ty3, ctx->tile_z, ctx->stream)
-                          : launch_step_fused<FLAGS>(f2, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0,
-                                                     ctx->variant == 2 ? ctx->tile_z : 0, ctx->stream);
+    e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0, ctx->variant == 2 ? ctx->tile_z : 0,
+                                 ctx->stream);
     time_mark(ctx);
-    ctx->fast_subcycles += (long long)ctx->ncell;
-    // the fix-up runs when cells can sub-cycle (cooling on) or, for variant 4, when there are sources
-    if (e != cudaSuccess || !((FLAGS & F_COOL) || (use4 && ctx->n_src > 0))) return e;
-    e = launch_step_fixup<FLAGS>(f2, ctx->g, sc, ctx->stream);
+    if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
     ctx->launches++;
+    fix_mark(ctx);
+    e = launch_step_fixup<FLAGS>(f, ctx->g, sc, scd, ctx->stream);
+    fix_mark(ctx);
     return e;
 }
 
-cudaError_t launch_step(aton_ctx *ctx, const StepConst &sc) {
-    const FieldsIO f = make_io(ctx);
+cudaError_t launch_step(aton_ctx *ctx, const StepConst &sc, const StepConstD &scd) {
+    const FieldsIO f = make_io(ctx, ctx->cur);
     ctx->launches++;
     switch (flags_of(ctx->p)) {
-        case 0: return launch_one<0>(ctx, f, sc);
-        case 1: return launch_one<1>(ctx, f, sc);
-        case 2: return launch_one<2>(ctx, f, sc);
-        case 3: return launch_one<3>(ctx, f, sc);
-        case 4: return launch_one<4>(ctx, f, sc);
-        case 5: return launch_one<5>(ctx, f, sc);
-        case 6: return launch_one<6>(ctx, f, sc);
-        default: return launch_one<7>(ctx, f, sc);
+        case 0: return launch_one<0>(ctx, f, sc, scd);
+        case 1: return launch_one<1>(ctx, f, sc, scd);
+        case 2: return launch_one<2>(ctx, f, sc, scd);
+        case 3: return launch_one<3>(ctx, f, sc, scd);
+        case 4: return launch_one<4>(ctx, f, sc, scd);
+        case 5: return launch_one<5>(ctx, f, sc, scd);
+        case 6: return launch_one<6>(ctx, f, sc, scd);
+        default: return launch_one<7>(ctx, f, sc, scd);
     }
 }
 
@@ -276,21 +341,27 @@ static int init_common(aton_t **out, const aton_grid_t *grid, const aton_box_t *
     if (ctx->p.max_sub == 0) ctx->p.max_sub = 1 << 14;
     ctx->dx = box->lx_cm / grid->nx;
     ctx->stream = (cudaStream_t)cuda_stream;
+    cudaGetDevice(&ctx->device);
     const size_t bytes = ctx->nalloc * sizeof(float);
     cudaError_t e = cudaSuccess;
     float **slots[11] = {&ctx->rad[0][0], &ctx->rad[0][1], &ctx->rad[0][2], &ctx->rad[0][3], &ctx->rad[1][0],
                          &ctx->rad[1][1], &ctx->rad[1][2], &ctx->rad[1][3], &ctx->x, &ctx->T, &ctx->nH};
     for (int i = 0; i < 11 && e == cudaSuccess; i++) e = cudaMalloc((void **)slots[i], bytes);
     for (int i = 0; i < 11 && e == cudaSuccess && slab; i++) e = cudaMemsetAsync(*slots[i], 0, bytes, ctx->stream);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, 3 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stats, N_STATS * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->partials, sizeof(double) * (REDUCE_BLOCKS + 1) * R_COUNT);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_mask, sizeof(unsigned) * (ctx->nalloc / 1024 + 1));
     const size_t defer_bytes = sizeof(unsigned) * (ctx->nalloc / 32 + 1);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->defer_mask, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->defer_mask, 0, defer_bytes, ctx->stream);
+    ctx->stiff_cap = (unsigned)std::max<size_t>(ctx->nalloc / 16, 4096);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stiff_q, sizeof(int) * (size_t)ctx->stiff_cap);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stiff_n, 2 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stiff_n, 0, 2 * sizeof(unsigned), ctx->stream);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->fixargs, 2 * sizeof(FixArgs));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_bits, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_bits, 0, defer_bytes, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stats, 0, N_STATS * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_mask, 0, sizeof(unsigned) * (ctx->nalloc / 1024 + 1), ctx->stream);
     if (e != cudaSuccess) {
         int code = fail(nullptr, e == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,
@@ -315,11 +386,14 @@ int aton_init_slab(aton_t **out, const aton_grid_t *global_grid, const aton_box_
 
 void aton_free(aton_t *ctx) {
     if (!ctx) return;
+    cudaSetDevice(ctx->device);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
     for (int b = 0; b < 2; b++)
         for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
     cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
-    cudaFree(ctx->src_mask); cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
+    cudaFree(ctx->src_mask); cudaFree(ctx->src_cell); cudaFree(ctx->src_rho); cudaFree(ctx->src_rho_d);
+    cudaFree(ctx->stiff_q); cudaFree(ctx->stiff_n); cudaFree(ctx->fixargs);
     cudaFree(ctx->stats); cudaFree(ctx->partials); cudaFree(ctx->defer_mask); cudaFree(ctx->src_bits);
     delete ctx;
 }
@@ -330,9 +404,9 @@ long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0;
 
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
-    if (variant < 0 || variant > 4) return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0..4");
-    if ((variant == 1 && !tiled_shape_ok(ctx->g, tile_y, tile_z)) || (variant == 2 && !fused_shape_ok(tile_y, tile_z)) ||
-        (variant == 3 && !v3_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)))
+    if (variant != 0 && variant != 2 && variant != 4)
+        return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0, 2 or 4");
+    if ((variant == 2 && !fused_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     return ATON_OK;
@@ -341,7 +415,9 @@ int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
 int aton_set_timing(aton_t *ctx, int on) {
     if (!ctx) return ATON_EINVAL;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
     ctx->ev.clear();
+    ctx->ev_fix.clear();
     ctx->timing = on != 0;
     return ATON_OK;
 }
@@ -357,6 +433,20 @@ int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches) {
     }
     *ms_total = tot;
     *n_launches = (long long)(ctx->ev.size() / 2);
+    return ATON_OK;
+}
+
+int aton_fixup_time(aton_t *ctx, double *ms_total, long long *n_launches) {
+    if (!ctx || !ms_total || !n_launches) return ATON_EINVAL;
+    CU(ctx, cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    for (size_t i = 0; i + 1 < ctx->ev_fix.size(); i += 2) {
+        float ms = 0.0f;
+        CU(ctx, cudaEventElapsedTime(&ms, ctx->ev_fix[i], ctx->ev_fix[i + 1]));
+        tot += ms;
+    }
+    *ms_total = tot;
+    *n_launches = (long long)(ctx->ev_fix.size() / 2);
     return ATON_OK;
 }
 
@@ -387,13 +477,15 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
             }
         }
     }
-    CU(ctx, cudaMemsetAsync(ctx->stats, 0, 3 * sizeof(unsigned long long), ctx->stream));
+    CU(ctx, cudaMemsetAsync(ctx->stats, 0, N_STATS * sizeof(unsigned long long), ctx->stream));
     double red[R_COUNT];
     int rc = run_reduce(ctx, false, red);
     if (rc) return rc;
     if (!(red[R_NHMIN] > 0.0) || !std::isfinite(red[R_M]))
         return fail(ctx, ATON_EINVAL, "aton_set_fields: n_H must be finite and > 0 everywhere (min %g)", red[R_NHMIN]);
     if (!ctx->mean_set) ctx->nH_mean = red[R_M] / (double)ctx->ncell;
+    ctx->fix_dirty = true;
+    CU(ctx, cudaMemsetAsync(ctx->stiff_n, 0, 2 * sizeof(unsigned), ctx->stream));
     ctx->steps_done = 0;
     ctx->fast_subcycles = 0;
     ctx->time_s = 0.0;
@@ -445,20 +537,25 @@ int aton_set_sources(aton_t *ctx, long long n, const float *pos, const double *r
     const size_t nwords = ctx->nalloc / 1024 + 1;
     std::vector<unsigned> mask(nwords, 0u);
     std::vector<float> rho(nu);
+    std::vector<double> rho_d(nu);
     const double inv_vol = 1.0 / (ctx->dx * ctx->dx * ctx->dx);
     for (size_t s = 0; s < nu; s++) {
         const unsigned seg = (unsigned)ucell[s] >> 5;
         mask[seg >> 5] |= 1u << (seg & 31);
-        rho[s] = (float)(urate[s] * inv_vol);
+        rho_d[s] = urate[s] * inv_vol;
+        rho[s] = (float)rho_d[s];
     }
     CU(ctx, cudaStreamSynchronize(ctx->stream));
-    cudaFree(ctx->src_cell); cudaFree(ctx->src_rho);
-    ctx->src_cell = nullptr; ctx->src_rho = nullptr; ctx->n_src = 0;
+    cudaFree(ctx->src_cell); cudaFree(ctx->src_rho); cudaFree(ctx->src_rho_d);
+    ctx->src_cell = nullptr; ctx->src_rho = nullptr; ctx->src_rho_d = nullptr; ctx->n_src = 0;
+    ctx->fix_dirty = true;
     CU(ctx, cudaMemcpyAsync(ctx->src_mask, mask.data(), sizeof(unsigned) * nwords, cudaMemcpyHostToDevice, ctx->stream));
     CU(ctx, cudaMemsetAsync(ctx->src_bits, 0, sizeof(unsigned) * (ctx->nalloc / 32 + 1), ctx->stream));
     if (nu > 0) {
         CU(ctx, cudaMalloc((void **)&ctx->src_cell, sizeof(int) * nu));
         CU(ctx, cudaMalloc((void **)&ctx->src_rho, sizeof(float) * nu));
+        CU(ctx, cudaMalloc((void **)&ctx->src_rho_d, sizeof(double) * nu));
+        CU(ctx, cudaMemcpyAsync(ctx->src_rho_d, rho_d.data(), sizeof(double) * nu, cudaMemcpyHostToDevice, ctx->stream));
         CU(ctx, cudaMemcpyAsync(ctx->src_cell, ucell.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, ctx->stream));
         CU(ctx, cudaMemcpyAsync(ctx->src_rho, rho.data(), sizeof(float) * nu, cudaMemcpyHostToDevice, ctx->stream));
         source_bits_kernel<<<(unsigned)((nu + 255) / 256), 256, 0, ctx->stream>>>(ctx->src_cell, (int)nu, ctx->src_bits);
@@ -488,8 +585,10 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     if (ctx->slab && n_steps > 1)
         return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first)");
     const StepConst sc = make_step_const(ctx, dt);
+    const StepConstD scd = make_step_const_d(ctx, dt);
+    if (n_steps > 0) CU(ctx, sync_fixargs(ctx, sc, scd, dt));
     for (int s = 0; s < n_steps; s++) {
-        CU(ctx, launch_step(ctx, sc));
+        CU(ctx, launch_step(ctx, sc, scd));
         ctx->cur = 1 - ctx->cur;
         ctx->steps_done++;
         ctx->time_s += dt;
@@ -502,6 +601,7 @@ int aton_set_mean_density(aton_t *ctx, double nH_mean) {
     if (!(nH_mean > 0.0) || !std::isfinite(nH_mean)) return fail(ctx, ATON_EINVAL, "aton_set_mean_density: must be > 0");
     ctx->nH_mean = nH_mean;
     ctx->mean_set = true;
+    ctx->fix_dirty = true;
     return ATON_OK;
 }
 
@@ -541,7 +641,7 @@ int aton_reduce_sums(aton_t *ctx, double *sums, int n) {
     double r[R_COUNT];
     int rc = run_reduce(ctx, true, r);
     if (rc) return rc;
-    unsigned long long st[3];
+    unsigned long long st[N_STATS];
     CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
     sums[0] = (double)ctx->ncell; sums[1] = r[R_X]; sums[2] = r[R_XM]; sums[3] = r[R_M]; sums[4] = r[R_N];
@@ -587,7 +687,7 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out) {
     double r[R_COUNT];
     int rc = run_reduce(ctx, true, r);
     if (rc) return rc;
-    unsigned long long st[3];
+    unsigned long long st[N_STATS];
     CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
     const double n = (double)ctx->ncell, cs = ctx->c * ctx->p.sigma_n;
@@ -604,6 +704,7 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out) {
     out->subcycles_total = (long long)st[0] + ctx->fast_subcycles;
     out->subcycles_max = std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
     out->cells_subcycled = (long long)st[2];
+    out->cells_fp64 = (long long)st[3];
     out->steps_done = ctx->steps_done;
     out->time_s = ctx->time_s;
     return ATON_OK;

@@ -150,7 +150,12 @@ __device__ __forceinline__ float clumping_i(float nH, const StepConst &c) {
 
 // ---------------------------------------------------------------- O4 chemistry / cooling
 // In/out: N, G (=F/c), x, T after transport + injection; nH fixed.  Returns the sub-cycle count.
-template <int FLAGS>
+// BAIL: give up (return -1, in/out values then meaningless) as soon as a sub-step is limited by the 10 % rule while
+// heating and cooling cancel to better than STIFF_KAPPA: the sub-step eps E/|H - Lambda| is then ill-conditioned
+// (the fp32 rate fits carry ~3e-6) and the caller redoes the cell with chemistry_f64 (aton_physics_f64.cuh).
+constexpr float STIFF_KAPPA = 1.0f / 64.0f;
+
+template <int FLAGS, bool BAIL = false>
 __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &gz, float &x, float &T,
                                          float nH, const StepConst &c) {
     constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL;
@@ -173,8 +178,12 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
         if (COOL) {
             // estimated net heating rate / (1.5 kB nH)  [K/s]
             float lamK = nH * (x * x * fmaf(CR, r.zrec, r.zff) + x * y * r.zxy) + c.compton0 * x * (T - c.t_cmb);
-            float ed = fabsf(y * N * heat_rate - lamK);
-            if (ed * t_left > c.eps_sub * theta) dts = c.eps_sub * theta / ed;
+            const float heat = y * N * heat_rate;
+            float ed = fabsf(heat - lamK);
+            if (ed * t_left > c.eps_sub * theta) {
+                if (BAIL && ed < STIFF_KAPPA * (heat + fabsf(lamK))) return -1;
+                dts = c.eps_sub * theta / ed;
+            }
         }
         // backward-Euler coupled (N, x) update, solved for delta = x' - x
         const float A = cs_nH * dts;

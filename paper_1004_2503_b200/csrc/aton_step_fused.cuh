@@ -1,6 +1,6 @@
-// Fused step kernel, variant 2 (the product kernel): transport + injection + chemistry in one pass that
-// reads every (N, G) value from HBM once, written for the issue-bound regime the first profile showed
-// (profiles/r01_a_step_tiled_512.md): ~2.5x fewer instructions per cell-update than variant 1.
+// Fused step kernel, variant 2: the FALLBACK for grids the product kernel (variant 4, aton_step_v4.cuh) cannot tile
+// (nx % 32 != 0 or ny % 4 != 0) and the home of the Quad / flux_row helpers variant 4 shares.  Transport + injection +
+// chemistry in one pass that reads every (N, G) value from HBM once (profiles/r01_b_step_fused_512.md).
 //
 // Decomposition:
 //  * one WARP per tile row of 128 cells: lane l owns the quad of cells 4l..4l+3 (one 128-bit access per
@@ -20,8 +20,9 @@
 //    cells that need sub-cycling are flagged in a bit mask and redone by step_fixup_kernel.
 // Algorithmic traffic: 7 reads + 6 writes of fp32 per cell-update = 52 B.
 #pragma once
+#include "aton_async.cuh"
 #include "aton_physics_pk.cuh"
-#include "aton_step_tiled.cuh"
+#include "aton_step_ref.cuh"
 
 namespace aton {
 
@@ -261,72 +262,6 @@ step_fused_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
     }
 }
 
-// ---------------------------------------------------------------------------------------------------
-// Fix-up: the cells flagged by the fused kernel hold their transported + injected (N, G) and their old
-// (x, T); run the sub-cycled operator Phi on them.  The mask is scanned in chunks of 256 words; flagged
-// cells are compacted into a shared-memory queue and processed one per thread once the queue holds a
-// few hundred (or the scan ends), so the data-dependent sub-cycle loops run on full warps.
-// stats[0] += sum(nsub - 1), stats[1] = max nsub, stats[2] += number of flagged cells.
-// ---------------------------------------------------------------------------------------------------
-constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS;
-
-template <int FLAGS>
-__global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(FieldsIO f, StepConst c, int nwords) {
-    __shared__ int queue[FIXUP_QCAP];
-    __shared__ int qn;
-    if (threadIdx.x == 0) qn = 0;
-    __syncthreads();
-    int nsub_extra = 0, nsub_max = 0, ncell = 0;
-    const int nchunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
-    for (int ch = blockIdx.x; ch < nchunks + (int)gridDim.x; ch += gridDim.x) {
-        const bool scan = ch < nchunks;         // the last trip only drains the queue
-        if (scan) {
-            const int w = ch * FIXUP_THREADS + threadIdx.x;
-            unsigned bits = w < nwords ? f.defer_mask[w] : 0u;
-            if (bits) {
-                f.defer_mask[w] = 0u;
-                int pos = atomicAdd(&qn, __popc(bits));
-                while (bits) {
-                    const int b = __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    queue[pos++] = w * 32 + b;
-                }
-            }
-        }
-        __syncthreads();
-        const int n = qn;
-        if (n >= FIXUP_QTHRESH || (!scan && n > 0)) {
-            for (int it = threadIdx.x; it < n; it += FIXUP_THREADS) {
-                const int id = queue[it];
-                float N = f.N1[id], gx = f.Gx1[id], gy = f.Gy1[id], gz = f.Gz1[id];
-                float x = f.x[id], T = f.T[id];
-                if (f.fix_inject && source_segment_flag(f, id)) N += source_lookup(f, id, c.dt);
-                const int ns = chemistry<FLAGS>(N, gx, gy, gz, x, T, __ldg(f.nH + id), c);
-                f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
-                f.x[id] = x; f.T[id] = T;
-                nsub_extra += ns - 1;
-                nsub_max = max(nsub_max, ns);
-                ncell++;
-            }
-            __syncthreads();
-            if (threadIdx.x == 0) qn = 0;
-        }
-        __syncthreads();
-        if (!scan) break;
-    }
-    // statistics: warp reduce, one atomic triple per warp that saw work
-    for (int o = 16; o > 0; o >>= 1) {
-        nsub_extra += __shfl_xor_sync(0xffffffffu, nsub_extra, o);
-        ncell += __shfl_xor_sync(0xffffffffu, ncell, o);
-        nsub_max = max(nsub_max, __shfl_xor_sync(0xffffffffu, nsub_max, o));
-    }
-    if ((threadIdx.x & 31) == 0 && ncell > 0) {
-        atomicAdd(f.stats, (unsigned long long)nsub_extra);
-        atomicMax(f.stats + 1, (unsigned long long)nsub_max);
-        atomicAdd(f.stats + 2, (unsigned long long)ncell);
-    }
-}
-
 inline int fused_default_lz(const Grid &g, int ty, int tile_z) {
     if (tile_z > 0) return tile_z < g.nz ? tile_z : g.nz;
     const long tiles_xy = (long)((g.nx / 4 + 31) / 32) * ((g.ny + ty - 1) / ty);
@@ -338,12 +273,9 @@ inline int fused_default_lz(const Grid &g, int ty, int tile_z) {
 template <int FLAGS, int TY>
 cudaError_t launch_step_fused_ty(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream) {
     using C = FusedCfg<TY>;
-    static bool attr_done = false;     // one per instantiation
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(step_fused_kernel<FLAGS, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    // per device, not per process: set it at every launch (a cheap driver call)
+    cudaError_t e = cudaFuncSetAttribute(step_fused_kernel<FLAGS, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
     const int lz = fused_default_lz(g, TY, tile_z);
     const dim3 grid((g.nx / 4 + 31) / 32, (g.ny + TY - 1) / TY, (g.nz + lz - 1) / lz);
     step_fused_kernel<FLAGS, TY><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz);
@@ -351,26 +283,15 @@ cudaError_t launch_step_fused_ty(const FieldsIO &f, const Grid &g, const StepCon
 }
 
 inline bool fused_shape_ok(int tile_y, int tile_z) {
-    return (tile_y == 0 || tile_y == 6 || tile_y == 8 || tile_y == 14) && tile_z >= 0;
+    return (tile_y == 0 || tile_y == 6 || tile_y == 14) && tile_z >= 0;
 }
 
-// one step = fused kernel, then (when the physics can sub-cycle, i.e. cooling is on) the fix-up kernel
+// one step = fused kernel, then (when the physics can sub-cycle, i.e. cooling is on) the fix-up kernel (aton_fixup.cuh)
 template <int FLAGS>
 cudaError_t launch_step_fused(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_y, int tile_z,
                               cudaStream_t stream) {
-    if (tile_y == 8) return launch_step_fused_ty<FLAGS, 8>(f, g, c, tile_z, stream);
     if (tile_y == 14) return launch_step_fused_ty<FLAGS, 14>(f, g, c, tile_z, stream);
     return launch_step_fused_ty<FLAGS, 6>(f, g, c, tile_z, stream);    // default: measured fastest
-}
-
-template <int FLAGS>
-cudaError_t launch_step_fixup(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream) {
-    const long ncell = (long)g.nx * g.ny * g.nz;
-    const int nwords = (int)((ncell + 31) / 32);
-    const int nchunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
-    const int blocks = nchunks < 148 * 8 ? nchunks : 148 * 8;
-    step_fixup_kernel<FLAGS><<<blocks, FIXUP_THREADS, 0, stream>>>(f, c, nwords);
-    return cudaGetLastError();
 }
 
 }  // namespace aton

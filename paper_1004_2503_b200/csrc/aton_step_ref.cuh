@@ -1,9 +1,9 @@
 // Reference step kernel (variant 0): one thread per cell, the 7-point stencil gathered straight from
 // global memory, closure recomputed for each neighbour, chemistry fused behind the transport update.
-// It is the simplest statement of the fused step on the device and the yardstick the tiled kernel
-// (aton_step_tiled.cuh) is compared with; it is also used for grids too small to tile.
+// It is the simplest statement of the fused step on the device: a cross-check for the product kernel
+// (aton_step_v4.cuh), never the default.
 #pragma once
-#include "aton_physics.cuh"
+#include "aton_physics_f64.cuh"
 
 namespace aton {
 
@@ -19,22 +19,34 @@ struct FieldsIO {
     const unsigned *src_mask;           // 1 bit per 32 consecutive cells: segment holds a source
     const int *src_cell;                // sorted flat cell indices of the sources
     const float *src_rho;               // rate / dx^3 per source cell [photons cm^-3 s^-1]
+    const double *src_rho_d;            // the same, unrounded (the fp64 redo of stiff cells)
     int n_src;
-    unsigned long long *stats;          // [0] += sub-cycles, [1] = max sub-cycles, [2] += cells redone by the fix-up
-    unsigned *defer_mask;               // variant 2+: 1 bit per cell, set = needs sub-cycling (fix-up kernel clears it)
+    unsigned long long *stats;          // [0] += sub-cycles beyond one per cell, [1] = max sub-cycles, [2] += cells redone,
+                                        // [3] += cells redone in fp64 (stiff)
+    unsigned *defer_mask;               // variant 2: 1 bit per cell, set = needs sub-cycling (fix-up kernel clears it)
     const unsigned *src_bits;           // variant 4: 1 bit per cell, set = the cell holds a source
-    int fix_inject;                     // variant 4: the fix-up kernel injects the sources (the step kernel did not)
+    int *stiff_q;                       // variant 4: [stiff_cap] ids of cells whose fp32 sub-cycling bailed out (they keep
+    unsigned *stiff_n;                  //   their transported values); [0] = ids queued this step (may exceed the cap)
+    unsigned stiff_cap;
 };
 
-// photons/cm^3 injected this step into flat cell `id` (0 for almost every cell) -- O3, NGP (L103)
-__device__ __forceinline__ float source_lookup(const FieldsIO &f, int id, float dt) {
+// index of flat cell `id` in the sorted source list, or -1 -- O3, NGP (L103)
+__device__ __forceinline__ int source_find(const FieldsIO &f, int id) {
     int lo = 0, hi = f.n_src;
     while (lo < hi) {
         int mid = (lo + hi) >> 1;
         if (__ldg(f.src_cell + mid) < id) lo = mid + 1; else hi = mid;
     }
-    if (lo < f.n_src && __ldg(f.src_cell + lo) == id) return __ldg(f.src_rho + lo) * dt;
-    return 0.0f;
+    return (lo < f.n_src && __ldg(f.src_cell + lo) == id) ? lo : -1;
+}
+// photons/cm^3 injected this step into flat cell `id` (0 for almost every cell)
+__device__ __forceinline__ float source_lookup(const FieldsIO &f, int id, float dt) {
+    const int s = source_find(f, id);
+    return s >= 0 ? __ldg(f.src_rho + s) * dt : 0.0f;
+}
+__device__ __forceinline__ double source_lookup_d(const FieldsIO &f, int id, double dt) {
+    const int s = source_find(f, id);
+    return s >= 0 ? __ldg(f.src_rho_d + s) * dt : 0.0;
 }
 
 __device__ __forceinline__ bool source_segment_flag(const FieldsIO &f, int id) {
@@ -62,7 +74,7 @@ __device__ __forceinline__ void add_neighbour(float sgn, float Nn, float gx, flo
 }
 
 template <int FLAGS>
-__global__ void __launch_bounds__(256) step_ref_kernel(FieldsIO f, Grid g, StepConst c) {
+__global__ void __launch_bounds__(256) step_ref_kernel(FieldsIO f, Grid g, StepConst c, StepConstD cd) {
     const int ncell = g.nx * g.ny * g.nz;
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
     int nsub = 0;
@@ -83,9 +95,9 @@ __global__ void __launch_bounds__(256) step_ref_kernel(FieldsIO f, Grid g, StepC
         float gx = fmaf(c.h, ax, c.keep * __ldg(f.Gx + id));
         float gy = fmaf(c.h, ay, c.keep * __ldg(f.Gy + id));
         float gz = fmaf(c.h, az, c.keep * __ldg(f.Gz + id));
-        if (source_segment_flag(f, id)) N += source_lookup(f, id, c.dt);
+        const double inj = source_segment_flag(f, id) ? source_lookup_d(f, id, cd.dt) : 0.0;
         float x = f.x[id], T = f.T[id];
-        nsub = chemistry<FLAGS>(N, gx, gy, gz, x, T, __ldg(f.nH + id), c);
+        nsub = phi_cell<FLAGS>(N, gx, gy, gz, x, T, __ldg(f.nH + id), inj, c, cd);
         f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
         f.x[id] = x; f.T[id] = T;
     }

@@ -1,9 +1,9 @@
 // Fused step kernel, variant 4 (the product kernel for grids with nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0
 // and ny % 2 == 0; the comments below describe the default 32 x 4 tile, WXQ = 8):
 // WARP-AUTONOMOUS tiles.  Transport + one chemistry sub-step in one pass over HBM (52 B per cell-update);
-// source cells and cells that need sub-cycling go to step_fixup_kernel.
+// source cells and cells that need sub-cycling are queued per warp and redone in batches (v4_fix_batch).
 //
-// Why: profiles/r01_c_step_v3_512.md -- in variant 3 every warp spends 20 % of its time spinning on the
+// Why: profiles/r01_c_step_v3_512.md -- with CTA-wide tiles every warp spent 20 % of its time spinning on the
 // per-plane CTA barrier (the slowest of 8 warps, its DRAM latency hiccups and the two edge warps' extra
 // halo row set the pace), 9 % on the source-mask load and 3 % in source binary searches, at 4 warps per
 // scheduler with nothing else to issue.  Here no warp ever waits for another warp:
@@ -19,12 +19,13 @@
 //    no source lookups -- the scheduler interleaves the chemistry's MUFU chains with the transport FMAs;
 //  * per-cell source flags come from a 1-bit-per-cell mask: a source cell is treated like a cell that
 //    needs sub-cycling (chemistry result discarded, flagged); the fix-up kernel injects and sub-cycles.
-// Arithmetic per cell is variant 3's (same order of operations): results are bit-identical to variant 3
-// except in source cells (scalar instead of packed chemistry there).
+//  * cells that need sub-cycling (and the source cells) are redone by the warp itself, 32 at a time, from a
+//    warp-private shared-memory queue (aton_fixup.cuh): their lines are still in L2 when the results land.
 #pragma once
 #include <type_traits>
 
-#include "aton_step_v3.cuh"
+#include "aton_fixup.cuh"
+#include "aton_step_fused.cuh"
 
 namespace aton {
 
@@ -40,7 +41,7 @@ struct V4Cfg {
     static constexpr int RAW_BUF = 4 * RAW_FIELD;        // [field][slot][RS]
     static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
     static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][WX]
-    static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN;
+    static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN + V4_QWORDS;   // + the warp's deferred-cell queue
     static constexpr int WARPS = ATON_V4_WARPS, THREADS = 32 * WARPS;
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
 };
@@ -89,7 +90,7 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
 #endif
 template <int FLAGS, int WXQ>
 __global__ void __launch_bounds__(V4Cfg<WXQ>::THREADS, ATON_V4_MINB)
-step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
+step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int zb, int ze) {
     using C = V4Cfg<WXQ>;
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -99,6 +100,10 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     float *raw = smem + warp * C::WARP_FLOATS;           // [2][4][6][RS], thread-private entries
     float *wyp = raw + 2 * C::RAW_BUF;                   // [4][4][32] plus terms
     float *wym = wyp + C::W_SIGN;                        //            minus terms
+    int *qi = reinterpret_cast<int *>(wym + C::W_SIGN);  // [V4_QCAP] ids of deferred cells + 4 statistics words
+    int qn = 0;                                          // ids queued (warp-uniform)
+    if (lane < 4) qi[V4_QCAP + lane] = 0;
+    __syncwarp();
 
     // planes [zb, ze) are advanced: the whole periodic grid (0, nz), or a slab's own planes (1, nz - 1) whose
     // ghost planes 0 and nz - 1 hold the neighbours' boundary planes (no wrap is ever taken then)
@@ -327,7 +332,15 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
             ATON_ST4(f.x, xs[0], xs[1]);
             ATON_ST4(f.T, Ts[0], Ts[1]);
 #undef ATON_ST4
-            if (nib) atomicOr(f.defer_mask + ((unsigned)oprev >> 5), nib << (oprev & 31));
+            if (__any_sync(0xffffffffu, nib != 0u)) {     // rare: queue the ids of the deferred cells
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const bool d = (nib >> j) & 1u;
+                    const unsigned bal = __ballot_sync(0xffffffffu, d);
+                    if (d) qi[qn + __popc(bal & ((1u << lane) - 1u))] = oprev + j;
+                    qn += __popc(bal);
+                }
+            }
         }
         // ---- y terms of plane m, written straight into the carried registers
         if (INPL) {
@@ -343,6 +356,10 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         } else {
             pend = t;
         }
+        if (FIN && qn >= 32) {                           // redo 32 deferred cells at a time (warp-uniform branch)
+            __syncwarp();                                // the stores of this and earlier planes are ordered before the redo
+            qn = v4_fix_drain<FLAGS>(fa, qi, qn, 32);
+        }
         oprev = ocur;
         kcur = kcur + 1 == g.nz ? 0 : kcur + 1;
         ocur = kcur * plane + rowoff;
@@ -356,6 +373,19 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     iter(yes, no, true, true);                 // m = 1: first own plane, nothing to finish yet
     while (m <= lzn) iter(yes, yes, true, true);   // steady state (the last one stages the z halo plane above)
     iter(no, yes, false, false);               // m = lzn + 1: z halo plane above, finishes plane lzn
+    if (qn > 0) {
+        __syncwarp();
+        v4_fix_drain<FLAGS>(fa, qi, qn, 1);
+    }
+    if (lane == 0) {
+        const int *wst = qi + V4_QCAP;
+        if (wst[2] > 0) {
+            atomicAdd(f.stats, (unsigned long long)wst[0]);
+            atomicMax(f.stats + 1, (unsigned long long)wst[1]);
+            atomicAdd(f.stats + 2, (unsigned long long)wst[2]);
+            if (wst[3] > 0) atomicAdd(f.stats + 3, (unsigned long long)wst[3]);
+        }
+    }
 }
 
 // tile shapes: 32 x 4 (nx % 32 == 0, ny % 4 == 0; the default: 13.8 ms per 1024^3 step) or 64 x 2 (nx % 64 == 0,
@@ -382,27 +412,24 @@ inline int v4_default_lz(const Grid &g, int tile_z, int nzr) {
 }
 
 template <int FLAGS, int WXQ>
-cudaError_t launch_step_v4_wxq(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream,
-                               int zb, int ze) {
+cudaError_t launch_step_v4_wxq(const FieldsIO &f, const Grid &g, const StepConst &c, const FixArgs *fa, int tile_z,
+                               cudaStream_t stream, int zb, int ze) {
     using C = V4Cfg<WXQ>;
-    static bool attr_done = false;     // one per instantiation
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS, WXQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    // the attribute is per device, not per process: set it at every launch (a cheap driver call)
+    cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS, WXQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
     const int lz = v4_default_lz<WXQ>(g, tile_z, ze - zb);
     const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (ze - zb + lz - 1) / lz);
-    step_v4_kernel<FLAGS, WXQ><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz, zb, ze);
+    step_v4_kernel<FLAGS, WXQ><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, fa, lz, zb, ze);
     return cudaGetLastError();
 }
 
-// wxq must come from v4_pick_wxq (non-zero)
+// wxq must come from v4_pick_wxq (non-zero); planes [zb, ze) are advanced
 template <int FLAGS>
-cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int wxq, int tile_z, cudaStream_t stream,
-                           int zb, int ze) {
-    if (wxq == 8) return launch_step_v4_wxq<FLAGS, 8>(f, g, c, tile_z, stream, zb, ze);
-    return launch_step_v4_wxq<FLAGS, 16>(f, g, c, tile_z, stream, zb, ze);
+cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, const FixArgs *fa, int wxq, int tile_z,
+                           cudaStream_t stream, int zb, int ze) {
+    if (wxq == 8) return launch_step_v4_wxq<FLAGS, 8>(f, g, c, fa, tile_z, stream, zb, ze);
+    return launch_step_v4_wxq<FLAGS, 16>(f, g, c, fa, tile_z, stream, zb, ze);
 }
 
 }  // namespace aton

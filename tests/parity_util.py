@@ -56,13 +56,16 @@ def max_rel_errors(g, st, c):
 
 
 def l1_errors(g, st, c):
-    """BASELINE.json full-run metric: relative L1 error per field (F measured against c*N)."""
+    """BASELINE.json full-run metric: relative L1 error per field.  F is given twice: "F" against c*sum N (reading
+    S16, the natural scale |F| <= cN) and "F_rel" against sum |F_ref| (the plain relative L1 of the flux itself)."""
     err = {}
     nsum = float(np.abs(st.N).sum())
     rel = lambda num: float(num / nsum) if nsum > 0 else (0.0 if num == 0 else float("inf"))   # dark region: exact zeros
     err["N"] = rel(np.abs(g["N"] - st.N).sum())
     dF = np.abs(g["Fx"] - st.Fx) + np.abs(g["Fy"] - st.Fy) + np.abs(g["Fz"] - st.Fz)
     err["F"] = rel(dF.sum() / c)
+    fsum = float((np.abs(st.Fx) + np.abs(st.Fy) + np.abs(st.Fz)).sum())
+    err["F_rel"] = float(dF.sum() / fsum) if fsum > 0 else (0.0 if dF.sum() == 0 else float("inf"))
     err["x"] = float(np.abs(g["x"] - st.x).sum() / np.abs(st.x).sum())
     err["T"] = float(np.abs(g["T"] - st.T).sum() / np.abs(st.T).sum())
     err["x_vol"] = float(abs(g["x"].astype(np.float64).mean() - st.x.mean()))

@@ -13,10 +13,15 @@ from parity_util import (gpu_run, l1_errors, max_rel_errors, oracle_run, state_t
 
 pytestmark = pytest.mark.gpu
 
+import os
+
 TOL_1STEP = 1e-4
 TOL_L1 = 1e-3
 TOL_XVOL = 1e-3
-VARIANTS = [0, 1, 2]
+# None = the library's default = the product kernel (variant 4) on every grid it can tile (all cases below but the
+# ragged 40^3 one, which the default runs through the variant-2 fallback); 0 and 2 are the cross-check kernels
+VARIANTS = [None, 0, 2]
+VIDS = ["default", "v0", "v2"]
 
 
 _cache = {}
@@ -40,15 +45,16 @@ def _oracle_cached(orc, w, n_steps):
 # workloads for the element-by-element checks: (builder, warm-up steps K, full-run steps)
 def _cases():
     return {
-        "cfg1_32": (lambda: wl.make_config(1), 60, 500),
-        "cfg2_twin48": (lambda: twin(2, 48, 120), 60, 120),
-        "cfg3_twin40": (lambda: twin(3, 40, 100), 50, 100),       # 40: several tiles + ragged tail
-        "cfg4_twin48": (lambda: twin(4, 48, 100), 50, 100),       # case A + clumping + coll. ion.
-        "cfg5_twin36": (lambda: twin(5, 36, 80), 40, 80),
+        "cfg1_32": (lambda: wl.make_config(1), 60, 500),           # config 1 itself, its full 500 steps
+        "cfg2_twin64": (lambda: twin(2, 64, 120), 60, 120),
+        "cfg3_twin64": (lambda: twin(3, 64, 100), 50, 100),
+        "cfg3_twin40": (lambda: twin(3, 40, 100), 50, 100),       # 40: not tileable by variant 4 -> fallback kernel, ragged tail
+        "cfg4_twin64": (lambda: twin(4, 64, 100), 50, 100),       # case A + clumping + coll. ion.
+        "cfg5_twin32": (lambda: twin(5, 32, 80), 40, 80),
     }
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 @pytest.mark.parametrize("case", list(_cases().keys()))
 def test_one_step_from_warm_state(orc, case, variant):
     """V2 / reading S17: both codes start from the oracle's state after K steps rounded to fp32."""
@@ -63,7 +69,7 @@ def test_one_step_from_warm_state(orc, case, variant):
         assert e <= TOL_1STEP, (case, variant, err)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 @pytest.mark.parametrize("case", list(_cases().keys()))
 def test_full_run(orc, case, variant):
     """V3: relative L1 per field <= 1e-3 and ionised volume fraction within 1e-3 after the run."""
@@ -74,7 +80,7 @@ def test_full_run(orc, case, variant):
     err = l1_errors(g, st, p.c)
     assert diag["n_nonfinite"] == 0 and diag["steps_done"] == n_steps
     assert err["x_vol"] <= TOL_XVOL, (case, err)
-    for f in ("N", "F", "x", "T"):
+    for f in ("N", "F", "F_rel", "x", "T"):
         assert err[f] <= TOL_L1, (case, variant, err)
     # diagnostics against the oracle's reduction of its own state
     d = orc.reduce(st, p)
@@ -87,7 +93,7 @@ def test_full_run(orc, case, variant):
     assert diag["subcycles_total"] == pytest.approx(st.sub_total, rel=0.02)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 def test_isothermal_and_no_collisions_switches(orc, variant):
     """The other physics-switch combinations (template instantiations) against the oracle."""
     for kw in (dict(cooling=0, coll_ion=0), dict(cooling=0, coll_ion=1, recomb_case=0),
@@ -95,7 +101,7 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
                dict(cooling=1, coll_ion=0, redshift=9.0),
                # paper-form clumping (Eq.15): C_R = K nH^0.7 and C_I = K' nH^0.2
                dict(cooling=1, coll_ion=1, recomb_case=0, clump_model=2, clump_a=300.0, clump_b=0.7, clump_i_a=8.0, clump_i_b=0.2)):
-        w = twin(3, 32, 60)
+        w = twin(3, 32, 60)                  # 32^3: the default runs the product kernel
         w.params.update(kw)
         ww = _warm(orc, w, 40)
         st, p = oracle_run(orc, ww, 1)
@@ -104,7 +110,7 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
         assert max(err.values()) <= TOL_1STEP, (kw, err)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 def test_reduce_matches_oracle(orc, variant):
     w = wl.synthetic_warm_state(twin(4, 32, 10))
     g, diag = gpu_run(w, 0, variant)
@@ -120,22 +126,52 @@ def test_reduce_matches_oracle(orc, variant):
     assert np.allclose(g["Fx"], w.Fx.numpy(), rtol=3e-7, atol=0)
 
 
-@pytest.mark.parametrize("variant", VARIANTS, ids=["v0", "v1", "v2"])
+@pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 def test_determinism_and_checkpoint(variant):
-    """V4: two runs are bit-identical; and because x, T, N round-trip exactly through get/set while
-    F = c*(F/c) does not, a restart matches to rounding (1e-6), not bitwise."""
-    w = wl.synthetic_warm_state(twin(4, 40, 10))
-    a, _ = gpu_run(w, 12, variant)
+    """V4: two runs are bit-identical, also when the steps are cut into several calls; and SURVEY 5's checkpoint:
+    run 2k steps == run k, aton_get_fields, aton_set_fields into a NEW context, run k.  n_H, x, T, N round-trip
+    bit-exactly; F does not (the device carries G = F/c: F -> fl(F/c) -> fl(c G) moves F by <= 2 ulp), so the resumed
+    run agrees to rounding, not bitwise: stated tolerance 2e-5 relative per field after k more steps (2 ulp of F
+    per restart, amplified by nothing: the scheme is a convex combination)."""
+    from paper_1004_2503_b200 import aton
+    w = wl.synthetic_warm_state(twin(4, 64, 10))
+    a, da = gpu_run(w, 12, variant)
     b, _ = gpu_run(w, 12, variant)
     for k in a:
         assert np.array_equal(a[k], b[k]), k
     c, _ = gpu_run(w, 12, variant, chunks=[5, 7])          # buffer parity across calls
     for k in a:
         assert np.array_equal(a[k], c[k]), k
+    # checkpoint / resume through the public calls
+    first = aton.from_workload(w)
+    if variant is not None:
+        first.set_kernel(variant)
+    first.step(w.dt, 6)
+    snap = first.get_fields(device="cpu")                  # the "snapshot every ~5000 steps" of PAPER.md:L411
+    d6 = first.reduce()
+    first.close()
+    second = aton.Aton(w.n, w.n, w.n, w.box_cm, w.params)
+    if variant is not None:
+        second.set_kernel(variant)
+    second.set_fields(*[snap[k].cuda() for k in ("nH", "x", "T", "N", "Fx", "Fy", "Fz")])
+    second.set_sources(w.src_pos.contiguous(), w.src_rate.contiguous())
+    again = second.get_fields(device="cpu")
+    for k in ("nH", "x", "T", "N"):
+        assert torch.equal(again[k], snap[k]), k           # exact round trip
+    assert torch.allclose(again["Fx"], snap["Fx"], rtol=3e-7, atol=0)
+    second.step(w.dt, 6)
+    r = {k: v.numpy() for k, v in second.get_fields(device="cpu").items()}
+    d12 = second.reduce()
+    second.close()
+    for k in ("N", "x", "T"):
+        assert np.allclose(r[k], a[k], rtol=2e-5, atol=0), k
+    for k in ("Fx", "Fy", "Fz"):
+        assert np.abs(r[k] - a[k]).max() <= 2e-5 * wl.C_CM_S * a["N"].max(), k
+    assert d12["steps_done"] == 6 and d6["steps_done"] == 6 and da["steps_done"] == 12
+    assert d12["x_vol"] == pytest.approx(da["x_vol"], rel=1e-6)
 
 
-@pytest.mark.parametrize("variant,tiles", [(1, ((4, 8), (8, 4), (2, 40), (16, 0))),
-                                           (2, ((6, 0), (14, 0), (8, 5), (6, 40), (14, 1)))], ids=["v1", "v2"])
+@pytest.mark.parametrize("variant,tiles", [(2, ((6, 0), (14, 0), (6, 5), (6, 40), (14, 1)))], ids=["v2"])
 def test_tile_shape_independence(variant, tiles):
     """V4: the tiled kernels' result does not depend on the tile shape (bitwise)."""
     w = wl.synthetic_warm_state(twin(5, 40, 10))
@@ -148,11 +184,11 @@ def test_tile_shape_independence(variant, tiles):
 
 
 def test_tiled_vs_reference_kernel():
-    """The three kernels differ only in rounding order (and, for variant 2, in which cells take the
-    sub-cycled path when the 10 % rule is decided within rounding: H5, continuous in the result)."""
-    w = wl.synthetic_warm_state(twin(4, 48, 10))
+    """The three kernels differ only in rounding order (and in which cells take the sub-cycled path when the 10 %
+    rule is decided within rounding: H5, continuous in the result)."""
+    w = wl.synthetic_warm_state(twin(4, 64, 10))
     a, da = gpu_run(w, 3, 0)
-    for variant in (1, 2):
+    for variant in (2, 4):
         b, db = gpu_run(w, 3, variant)
         for k in ("N", "x", "T"):
             assert np.allclose(a[k], b[k], rtol=5e-5, atol=0), (variant, k)
@@ -160,17 +196,23 @@ def test_tiled_vs_reference_kernel():
         assert db["subcycles_max"] == da["subcycles_max"]
 
 
-def test_fixup_path_statistics():
-    """Variant 2: cells that need sub-cycling are redone by the fix-up kernel, counted, and the mask is
-    left clean (a second identical context gives the same counts; an isothermal run never defers)."""
+@pytest.mark.parametrize("variant", [2, 4], ids=["v2", "v4"])
+def test_fixup_path_statistics(variant):
+    """Cells that need sub-cycling are redone (variant 4: by the producing warp; variant 2: by the fix-up kernel),
+    counted, and nothing is left queued (a second identical context gives the same counts); an isothermal run never
+    sub-cycles (variant 4 still redoes its one source cell per step)."""
     w = wl.make_config(1)
-    g, d = gpu_run(w, 40, 2)
+    g, d = gpu_run(w, 40, variant)
     assert d["cells_subcycled"] > 0 and d["subcycles_max"] > 1
     assert d["subcycles_total"] > 40 * w.n ** 3
+    assert 0 <= d["cells_fp64"] <= d["cells_subcycled"]
+    g1, d1 = gpu_run(w, 40, variant)
+    assert all(d1[k] == d[k] for k in ("cells_subcycled", "subcycles_total", "subcycles_max", "cells_fp64"))
     w2 = wl.make_config(1)
     w2.params.update(cooling=0)
-    g2, d2 = gpu_run(w2, 10, 2)
-    assert d2["cells_subcycled"] == 0 and d2["subcycles_max"] == 1 and d2["subcycles_total"] == 10 * w.n ** 3
+    g2, d2 = gpu_run(w2, 10, variant)
+    assert d2["cells_subcycled"] == (10 if variant == 4 else 0) and d2["cells_fp64"] == 0
+    assert d2["subcycles_max"] == 1 and d2["subcycles_total"] == 10 * w.n ** 3
 
 
 def test_non_cubic_grid_and_source_edges(orc):
@@ -187,7 +229,7 @@ def test_non_cubic_grid_and_source_edges(orc):
                     [1.0 / 24 * 3, 0.3, 0.2], [1.0, 0.0, 0.0]], np.float32)
     rate = np.array([1e50, 2e50, 3e50, 1e50, 5e49, 7e49])
     dt = wl.courant_dt(dx)
-    for variant in VARIANTS + [3, 4]:         # 3 and 4 cannot tile 24 x 10: they run the variant-2 kernel
+    for variant in (0, 2, 4):                 # 4 cannot tile 24 x 10: it runs the variant-2 kernel
         a = aton.Aton(nx, ny, nz, dx * nx, p)
         a.set_kernel(variant)
         a.set_fields(*[torch.from_numpy(v).cuda() for v in (nH, x, T)])
@@ -229,6 +271,9 @@ def test_api_errors():
     d = a.reduce()
     assert d["steps_done"] == 2 and d["time_s"] == pytest.approx(2 * a.courant_dt(0.8))
     assert a.launch_count() > 0
+    for gone in (1, 3, 5, -1):
+        with pytest.raises(aton.AtonError):
+            a.set_kernel(gone)                                            # round 1's variants 1 and 3 no longer exist
     a.close()
 
 
@@ -251,9 +296,8 @@ def test_empty_sources_and_vacuum_conservation():
 
 
 # ------------------------------------------------------------------------------------------------
-# Variant 3 (full-tile kernel: nx % 128 == 0, ny % tile_y == 0).  The cubic twins above are too small
-# for it (they run the variant-2 kernel under the default variant), so it gets non-cubic grids whose
-# x extent spans one or two 128-cell tiles, several y tiles and a ragged z chunk.
+# Non-cubic grids for the product kernel: x extents of one to eight 32-cell warp tiles (ragged last CTA), several y
+# tiles, ragged z chunks, sources on tile corners / edges and across every periodic seam.
 # ------------------------------------------------------------------------------------------------
 def _slab_case(nx, ny, nz, flags7, seed, paper_clumping=False):
     """Random log-normal-ish density on an (nz, ny, nx) grid, sources on tile corners / edges, physics of
@@ -292,10 +336,9 @@ def _run_slab(variant, tile, nH, x, T, p, dx, pos, rate, n_steps, rad=None):
 
 
 @pytest.mark.parametrize("variant,shape,flags7",
-                         [(3, (128, 16, 11), True), (3, (256, 24, 9), False), (3, (128, 8, 3), True),
-                          (4, (128, 16, 11), True), (4, (256, 24, 9), False), (4, (32, 8, 5), True),
+                         [(4, (128, 16, 11), True), (4, (256, 24, 9), False), (4, (32, 8, 5), True),
                           (4, (160, 12, 1), True), (4, (64, 4, 70), False), (4, (96, 8, 7), "paper")],
-                         ids=["v3_128x16x11_A", "v3_256x24x9_B", "v3_128x8x3_A", "v4_128x16x11_A", "v4_256x24x9_B",
+                         ids=["v4_128x16x11_A", "v4_256x24x9_B",
                               "v4_32x8x5_A", "v4_160x12x1_A", "v4_64x4x70_B", "v4_96x8x7_paper_clumping"])
 def test_full_tile_kernels_against_oracle(orc, variant, shape, flags7):
     nx, ny, nz = shape
@@ -314,15 +357,14 @@ def test_full_tile_kernels_against_oracle(orc, variant, shape, flags7):
     warm = [np.ascontiguousarray(v, dtype=np.float32) for v in (st.x, st.T, st.N, st.Fx, st.Fy, st.Fz)]
     st1 = orc.State(nH, *warm)
     orc.step(st1, op, dt, 1, pos.astype(np.float64), rate)
-    tiles = ((0, 0), (4, 2), (8, 5)) + (((16, 0),) if ny % 16 == 0 else ()) if variant == 3 else ((0, 0), (0, 1), (4, 3), (4, 64)) + (((2, 0), (2, 5)) if nx % 64 == 0 else ())
+    tiles = ((0, 0), (0, 1), (4, 3), (4, 64)) + (((2, 0), (2, 5)) if nx % 64 == 0 else ())
     for tile in tiles:
         g1, d1 = _run_slab(variant, tile, nH, warm[0], warm[1], p, dx, pos, rate, 1, rad=warm[2:])
         e1 = max_rel_errors(g1, st1, op.c)
         assert max(e1.values()) <= TOL_1STEP, (tile, e1)
 
 
-@pytest.mark.parametrize("variant,tiles", [(3, ((0, 0), (4, 0), (16, 0), (8, 3), (16, 13), (4, 1))),
-                                           (4, ((0, 0), (0, 1), (2, 2), (4, 0), (4, 5), (2, 13)))], ids=["v3", "v4"])
+@pytest.mark.parametrize("variant,tiles", [(4, ((0, 0), (0, 1), (2, 2), (4, 0), (4, 5), (2, 13)))], ids=["v4"])
 def test_full_tile_kernels_tile_shape_independence_determinism_and_v2_agreement(variant, tiles):
     nH, x, T, p, dx, pos, rate = _slab_case(256, 32, 13, True, seed=5)
     ref, dref = _run_slab(variant, (0, 0), nH, x, T, p, dx, pos, rate, 25)
@@ -339,18 +381,6 @@ def test_full_tile_kernels_tile_shape_independence_determinism_and_v2_agreement(
     assert d2["subcycles_total"] == pytest.approx(dref["subcycles_total"], rel=1e-3)
 
 
-def test_v4_equals_v3_bitwise_without_sources():
-    """Variant 4 keeps variant 3's order of operations per cell; only source cells take another path."""
-    nH, x, T, p, dx, pos, rate = _slab_case(128, 16, 9, True, seed=3)
-    w = wl.synthetic_warm_state(twin(4, 128, 1))            # realizable radiation field to cut a slab from
-    rad = [w.x.numpy()[:9, :16, :], w.T.numpy()[:9, :16, :]] + [t.numpy()[:9, :16, :] for t in (w.N, w.Fx, w.Fy, w.Fz)]
-    none = (np.zeros((0, 3), np.float32), np.zeros(0))
-    a, _ = _run_slab(3, (0, 0), nH, rad[0], rad[1], p, dx, *none, 5, rad=rad[2:])
-    b, _ = _run_slab(4, (0, 0), nH, rad[0], rad[1], p, dx, *none, 5, rad=rad[2:])
-    for k in a:
-        assert np.array_equal(a[k], b[k]), k
-
-
 # ------------------------------------------------------------------------------------------------
 # BASELINE.json's full size (config 5, 1024^3) in the launch configuration bench.py times (default
 # kernel variant and tile shape).  The oracle cannot run 2^30 cells, but the scheme's domain of
@@ -359,7 +389,18 @@ def test_v4_equals_v3_bitwise_without_sources():
 # the full-grid GPU run.  Both codes start from generator output only (dark start, or
 # workloads.synthetic_warm_state): no oracle input comes from the CUDA path.
 # ------------------------------------------------------------------------------------------------
+def _subcube_sources(w, org, size):
+    """Sources of the full grid that fall inside the periodic sub-cube at `org`, as (positions in sub-cube units, rates)."""
+    n = w.n
+    src_cell = torch.floor(w.src_pos.double() * n).long() % n           # (ns, 3) as (i, j, k)
+    rel = (src_cell - torch.tensor(org)) % n
+    inside = (rel < size).all(dim=1)
+    return ((rel[inside].double() + 0.5) / size).numpy(), w.src_rate[inside].numpy()
+
+
 def _subcube_check(orc, w, state_name, origins, m, p_steps, nH_mean):
+    """p_steps of the full grid on the GPU against the oracle on (m + 2 p_steps)^3 sub-cubes: relative L1 of the inner
+    m^3 (BASELINE.json's full-run metric; the per-cell 1-step bar is _onestep_check's job)."""
     from paper_1004_2503_b200 import aton
     n, size = w.n, m + 2 * p_steps
     a = aton.from_workload(w)
@@ -368,16 +409,12 @@ def _subcube_check(orc, w, state_name, origins, m, p_steps, nH_mean):
     diag = a.reduce()
     a.close()
     assert diag["n_nonfinite"] == 0 and diag["steps_done"] == p_steps
-    src_cell = torch.floor(w.src_pos.double() * n).long() % n           # (ns, 3) as (i, j, k)
     worst = {}
     for org in origins:
         cut = {k: wl.cut_subcube(getattr(w, k), org, size).numpy() for k in ("nH", "x", "T", "N", "Fx", "Fy", "Fz")}
         st = orc.State(*[cut[k] for k in ("nH", "x", "T", "N", "Fx", "Fy", "Fz")])
         op = orc.make_params(w.params, w.dx, nH_mean)
-        rel = (src_cell - torch.tensor(org)) % n                         # sources inside the sub-cube
-        inside = (rel < size).all(dim=1)
-        pos = ((rel[inside].double() + 0.5) / size).numpy()
-        rate = w.src_rate[inside].numpy()
+        pos, rate = _subcube_sources(w, org, size)
         orc.step(st, op, w.dt, p_steps, pos, rate)
         sl = slice(p_steps, p_steps + m)
         inner_org = tuple(o + p_steps for o in org)
@@ -386,30 +423,101 @@ def _subcube_check(orc, w, state_name, origins, m, p_steps, nH_mean):
         err = l1_errors(g, ref, op.c)
         for k, e in err.items():
             worst[k] = max(worst.get(k, 0.0), e)
-        assert max(err[k] for k in ("N", "F", "x", "T")) <= TOL_L1, (state_name, org, int(inside.sum()), err)
-        # cell by cell (8 fp32 steps; 1e-4 is the 1-step bar from an oracle-evolved state): at most 0.2 % of
-        # the cells beyond 1e-3 in x and T, 5 % in N (8 steps after a dark start the whole front is leading edge).  Those few are (i) extreme-density source cells (n_H ~ 1 cm^-3, C_R ~ 1e4,
-        # 50-70 sub-cycles per step) where heating and cooling nearly cancel, so the 10 % rule's sub-step
-        # eps E/|H - Lambda| is ill-conditioned and the fp32 and fp64 sub-step sequences separate at the
-        # truncation level of the first-order sub-step (per cent), and (ii) leading-edge cells of a front,
-        # where the upwind difference N - G_d cancels (H4/H5).  The reference kernel (variant 0)
-        # shows the same errors in the same cells: they belong to the fp32 formulation, not to the tiling.
-        big = ref.N > 1e-20 * max(ref.N.max(), 1e-300)
-        rel = {"x": np.abs(g["x"] - ref.x) / ref.x, "T": np.abs(g["T"] - ref.T) / ref.T}
-        if big.any():
-            rel["N"] = np.abs(g["N"][big] - ref.N[big]) / ref.N[big]
-        for k, e in rel.items():
-            assert np.mean(e > 1e-3) <= (5e-2 if k == "N" else 2e-3) and e.max() <= 0.5, (state_name, org, k, e.max(), float(np.mean(e > 1e-3)))
-    return worst
+        assert max(err[k] for k in ("N", "F", "x", "T")) <= TOL_L1, (state_name, org, len(rate), err)
+    return worst, diag
+
+
+def _paste_subcube(dst, src, org):
+    """dst[z0:z0+s, y0:y0+s, x0:x0+s] = src, periodic; dst on the GPU, src a numpy array."""
+    n, s = dst.shape[0], src.shape[0]
+    x0, y0, z0 = org
+    iz = (torch.arange(s, device=dst.device) + z0) % n
+    iy = (torch.arange(s, device=dst.device) + y0) % n
+    ix = (torch.arange(s, device=dst.device) + x0) % n
+    dst[iz[:, None, None], iy[None, :, None], ix[None, None, :]] = torch.from_numpy(np.ascontiguousarray(src, dtype=np.float32)).to(dst.device)
+
+
+def _onestep_check(orc, w, origins, size, k_warm, nH_mean):
+    """The north_star's 1-step bar at full size, in the bench's launch configuration: max relative error <= 1e-4 on
+    N, F, x, T (where N > 1e-20 max N) after ONE step.  Two kinds of start, both made without the CUDA path:
+      (a) oracle-evolved: each `size`^3 sub-cube of the dark full-size workload (its density, its sources) is evolved
+          k_warm steps by the oracle as a small periodic box, rounded to fp32 and pasted into the full-size state;
+      (b) the generator's synthetic warm state everywhere else (far from equilibrium: the heaviest sub-cycling).
+    The GPU advances the WHOLE grid one step with the default kernel; the oracle advances each sub-cube one step;
+    the cells whose stencil stays inside the sub-cube (the inner (size-2)^3) are compared one by one."""
+    from paper_1004_2503_b200 import aton
+    op = orc.make_params(w.params, w.dx, nH_mean)
+    ww = wl.synthetic_warm_state(w)
+    names = ("x", "T", "N", "Fx", "Fy", "Fz")
+    for org in origins[0::2]:                                           # (a): evolve from the dark start, paste
+        cut = {k: wl.cut_subcube(getattr(w, k), org, size).numpy() for k in ("nH",) + names}
+        st = orc.State(*[cut[k] for k in ("nH",) + names])
+        pos, rate = _subcube_sources(w, org, size)
+        orc.step(st, op, w.dt, k_warm, pos, rate)
+        for k in names:
+            _paste_subcube(getattr(ww, k), getattr(st, k), org)
+    refs = []
+    for org in origins:                                                 # both kinds: one oracle step from what the GPU gets
+        cut = {k: wl.cut_subcube(getattr(ww, k), org, size).numpy() for k in ("nH",) + names}
+        st = orc.State(*[cut[k] for k in ("nH",) + names])
+        pos, rate = _subcube_sources(w, org, size)
+        orc.step(st, op, w.dt, 1, pos, rate)
+        refs.append((org, st, cut, len(rate)))
+    a = aton.from_workload(ww)
+    del ww
+    torch.cuda.empty_cache()
+    a.step(w.dt, 1)
+    out = a.get_fields(device="cuda", names=names)
+    diag = a.reduce()
+    a.close()
+    assert diag["n_nonfinite"] == 0 and diag["steps_done"] == 1
+    worst = {}
+    sl = slice(1, size - 1)
+    bad = []
+    for org, st, cut, nsrc in refs:
+        g = {k: wl.cut_subcube(out[k], tuple(o + 1 for o in org), size - 2).numpy() for k in names}
+        ref = type("S", (), {k: getattr(st, k)[sl, sl, sl] for k in names})
+        err = max_rel_errors(g, ref, op.c)
+        for k, e in err.items():
+            worst[k] = max(worst.get(k, 0.0), e)
+        if max(err.values()) > TOL_1STEP:                              # name the worst cells: start state -> both results
+            big = ref.N > 1e-20 * ref.N.max()
+            for k in ("x", "T", "N"):
+                e = np.abs(g[k] - getattr(ref, k)) / np.maximum(np.abs(getattr(ref, k)), 1e-300)
+                if k == "N":
+                    e = np.where(big, e, 0.0)
+                for idx in np.argsort(e.ravel())[::-1][:3]:
+                    kk, jj, ii = np.unravel_index(idx, e.shape)
+                    if e[kk, jj, ii] > TOL_1STEP:
+                        c0 = {f: float(cut[f][kk + 1, jj + 1, ii + 1]) for f in ("nH", "x", "T", "N")}
+                        bad.append((org, nsrc, k, float(e[kk, jj, ii]), c0,
+                                    {f: (float(g[f][kk, jj, ii]), float(getattr(ref, f)[kk, jj, ii])) for f in ("x", "T", "N")}))
+            bad.append((org, nsrc, "max-rel", err, int(st.sub_max)))
+    assert not bad, bad
+    return worst, diag
 
 
 def _have_hbm(gb):
     return torch.cuda.is_available() and torch.cuda.get_device_properties(0).total_memory >= gb * 1e9
 
 
+def _origins(w, size):
+    """Sub-cubes: around the two brightest sources, across the periodic corner, across CTA / tile seams, a void."""
+    n = w.n
+    cells = (torch.floor(w.src_pos.double() * n).long() % n)
+    top = torch.argsort(w.src_rate, descending=True)[:2]
+    half = size // 2
+    origins = [tuple(int(v) for v in ((cells[s] - half) % n)) for s in top]
+    origins += [(n - 20, n - 20, n - 20), (128 - 20, 4 * 37 - 20, 64 - 20)]
+    flat = int(torch.argmin(w.nH.reshape(-1)[: n * n * 64]))
+    origins.append(tuple(int(v) for v in ((torch.tensor([flat % n, (flat // n) % n, flat // (n * n)]) - half) % n)))
+    return origins
+
+
 @pytest.mark.parametrize("cfg", [3, 4, 5])
 def test_full_size_configs_on_subcubes_against_oracle(orc, cfg):
-    """Configs 3 (256^3), 4 (512^3) and 5 (1024^3) at BASELINE.json's full grid sizes, default kernel and tile."""
+    """Configs 3 (256^3), 4 (512^3) and 5 (1024^3) at BASELINE.json's full grid sizes, default kernel and tile:
+    8 steps from the dark start and from the synthetic warm state, relative L1 on sub-cubes."""
     n = {3: 256, 4: 512, 5: 1024}[cfg]
     if not _have_hbm(150 if cfg == 5 else 30):
         pytest.skip("needs the full working set in HBM (about 110 GB for 1024^3)")
@@ -417,33 +525,54 @@ def test_full_size_configs_on_subcubes_against_oracle(orc, cfg):
     w = wl.make_config(cfg, device="cuda")
     assert w.n == n
     nH_mean = float(w.nH.double().mean())
-    # sub-cubes: around the two brightest sources, across the periodic corner, across CTA / tile seams, a void
-    cells = (torch.floor(w.src_pos.double() * n).long() % n)
-    top = torch.argsort(w.src_rate, descending=True)[:2]
-    half = (m + 2 * p_steps) // 2
-    origins = [tuple(int(v) for v in ((cells[s] - half) % n)) for s in top]
-    origins += [(n - 20, n - 20, n - 20), (128 - 20, 4 * 37 - 20, 64 - 20)]
-    flat = int(torch.argmin(w.nH.reshape(-1)[: n * n * 64]))
-    origins.append(tuple(int(v) for v in ((torch.tensor([flat % n, (flat // n) % n, flat // (n * n)]) - half) % n)))
-    dark = _subcube_check(orc, w, "dark", origins, m, p_steps, nH_mean)
+    origins = _origins(w, m + 2 * p_steps)
+    dark, _ = _subcube_check(orc, w, "dark", origins, m, p_steps, nH_mean)
     ww = wl.synthetic_warm_state(w)
     del w
     torch.cuda.empty_cache()
-    warm = _subcube_check(orc, ww, "warm", origins, m, p_steps, nH_mean)
-    print(f"config {cfg}: worst relative L1 on sub-cubes: dark", dark, "warm", warm)
+    warm, dw = _subcube_check(orc, ww, "warm", origins, m, p_steps, nH_mean)
+    print(f"config {cfg}: worst relative L1 on sub-cubes: dark", dark, "warm", warm, "fp64 cells", dw["cells_fp64"])
 
 
-def test_config2_full_grid_against_oracle(orc):
-    """Config 2 at its full 128^3 grid (default kernel: variant 4): 150 of its 1000 steps against the oracle run on
-    the whole grid -- BASELINE.json's full-run metric."""
-    w = wl.make_config(2)
-    assert w.n == 128 and w.n_steps == 1000
-    steps = 150
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_one_step_bar(orc, cfg):
+    """The 1-step bar (max relative error 1e-4, cell by cell) at the full grid sizes of configs 3-5."""
+    n = {3: 256, 4: 512, 5: 1024}[cfg]
+    if not _have_hbm(150 if cfg == 5 else 30):
+        pytest.skip("needs the full working set in HBM (about 110 GB for 1024^3)")
+    w = wl.make_config(cfg, device="cuda")
+    assert w.n == n
+    size = 40
+    worst, diag = _onestep_check(orc, w, _origins(w, size), size, 16, float(w.nH.double().mean()))
+    print(f"config {cfg}: worst 1-step max-rel errors on sub-cubes", worst, "cells redone", diag["cells_subcycled"],
+          "in fp64", diag["cells_fp64"], "max sub-cycles", diag["subcycles_max"])
+
+
+def _full_run(orc, w, steps):
     st, p = oracle_run(orc, w, steps)
     g, diag = gpu_run(w, steps)
     err = l1_errors(g, st, p.c)
     assert diag["n_nonfinite"] == 0 and diag["steps_done"] == steps
-    assert err["x_vol"] <= TOL_XVOL and max(err[k] for k in ("N", "F", "x", "T")) <= TOL_L1, err
+    assert err["x_vol"] <= TOL_XVOL and max(err[k] for k in ("N", "F", "F_rel", "x", "T")) <= TOL_L1, err
     d = orc.reduce(st, p)
     assert diag["x_mass"] == pytest.approx(d["x_mass"], abs=2e-3) and diag["photons_total"] == pytest.approx(d["photons_total"], rel=2e-3)
     assert diag["subcycles_total"] == pytest.approx(st.sub_total, rel=0.02)
+    return err, diag
+
+
+def test_config2_full_run_against_oracle(orc):
+    """Config 2 in full: its 128^3 grid, all of its 1000 steps, default kernel (variant 4), against the oracle run on
+    the whole grid (about 100 s of oracle on 16 cores) -- BASELINE.json's full-run metric."""
+    w = wl.make_config(2)
+    assert w.n == 128 and w.n_steps == 1000
+    err, diag = _full_run(orc, w, w.n_steps)
+    print("config 2, 1000 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
+
+
+@pytest.mark.skipif(os.environ.get("ATON_SLOW", "") != "1", reason="config 3 in full is ~30 min of oracle: set ATON_SLOW=1")
+def test_config3_full_run_against_oracle(orc):
+    """Config 3 in full: 256^3, 2000 steps (opt-in; the result of the round's run is recorded in DESIGN.md)."""
+    w = wl.make_config(3)
+    assert w.n == 256 and w.n_steps == 2000
+    err, diag = _full_run(orc, w, w.n_steps)
+    print("config 3, 2000 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
