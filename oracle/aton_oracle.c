@@ -55,6 +55,7 @@ typedef struct {
     int coll_ion;        /* collisional ionisation on/off */
     int clump_model;     /* 0 none; 1: C=max(1,a+b*delta); 2: C=max(1,a*nH^b) */
     int max_sub;         /* sub-cycle cap (S18) */
+    int flux;            /* intercell flux: 0 Lax-Friedrichs (the one the paper used), 1 HLL */
 } orc_params;
 
 typedef struct {          /* T-dependent coefficients, reading S7 (Hui & Gnedin 1997; Cen 1992) */
@@ -151,6 +152,85 @@ void orc_transport(int nx, int ny, int nz, const double *N, const double *Fx, co
                         double f_lo = 0.5 * (gm[v] + g0[v]) - 0.5 * c * (U[v] - Um[v]);  /* i-1/2 */
                         Un[v] -= dt / dx * (f_hi - f_lo);                                /* Eq.A2 */
                     }
+                }
+                N1[id] = Un[0]; Fx1[id] = Un[1]; Fy1[id] = Un[2]; Fz1[id] = Un[3];
+            }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O2' transport with the HLL intercell flux ("the code is able to evaluate intercell fluxes using
+ * both the ... HLL or the simpler Lax-Friedrich scheme"; reading S20).  The paper prints
+ * neither the flux nor the wave speeds; the standard Harten-Lax-van Leer form for the M1 system is taken:
+ *     FF_{i+1/2} = [ l+ FF_i - l- FF_{i+1} + l+ l- (U_{i+1} - U_i) ] / (l+ - l-),
+ *     l+ = max(0, lmax_i, lmax_{i+1}),   l- = min(0, lmin_i, lmin_{i+1}),
+ * with lmin, lmax the extreme eigenvalues of the Jacobian d FF_d / d U of the M1 flux function in the direction d
+ * of the face.  For the Levermore closure they have the closed form (in units of c; mu = F_d/|F|, xi = sqrt(4-3f^2))
+ *     l(+-) = [ mu f +- sqrt( (2/3)(xi^2 - xi) + 2 mu^2 (2 - f^2 - xi) ) ] / xi
+ * (pinned in tests/test_oracle_hll.py against numpy's eigenvalues of the finite-difference Jacobian of flux_fn).
+ * With l+ = -l- = c the flux is the Lax-Friedrichs flux of orc_transport.
+ * ------------------------------------------------------------------------------------------- */
+void orc_m1_wavespeeds(double N, const double F[3], double c, int d, double *lmin, double *lmax) {
+    double Fn = sqrt(F[0] * F[0] + F[1] * F[1] + F[2] * F[2]);
+    double f = 0.0, mu = 0.0;
+    if (N > 0.0) {
+        f = Fn / (c * N);
+        if (f > 1.0) f = 1.0;
+    }
+    if (Fn > 0.0) mu = F[d] / Fn;
+    double xi = sqrt(4.0 - 3.0 * f * f);
+    double disc = (2.0 / 3.0) * (xi * xi - xi) + 2.0 * mu * mu * (2.0 - f * f - xi);
+    double root = sqrt(disc > 0.0 ? disc : 0.0);
+    *lmin = c * (mu * f - root) / xi;
+    *lmax = c * (mu * f + root) / xi;
+}
+
+/* physical flux through a face normal to axis d (the oracle's own flux_fn, exported for the Jacobian pin) */
+void orc_flux_fn(int d, double N, const double F[3], double c, double out[4]) { flux_fn(d, N, F, c, out); }
+
+/* HLL flux between a left state (Ul, flux gl) and a right state (Ur, gr) with signal speeds sm <= 0 <= sp */
+void orc_hll_flux(const double Ul[4], const double gl[4], const double Ur[4], const double gr[4], double sm,
+                  double sp, double out[4]) {
+    for (int v = 0; v < 4; v++) {
+        if (sp - sm > 0.0) out[v] = (sp * gl[v] - sm * gr[v] + sp * sm * (Ur[v] - Ul[v])) / (sp - sm);
+        else out[v] = 0.5 * (gl[v] + gr[v]);       /* both states are beams across the face: nothing crosses it */
+    }
+}
+
+static void hll_face(int d, const double Ul[4], const double Ur[4], double c, double out[4]) {
+    double gl[4], gr[4], a, b, sm = 0.0, sp = 0.0;
+    flux_fn(d, Ul[0], Ul + 1, c, gl);
+    flux_fn(d, Ur[0], Ur + 1, c, gr);
+    orc_m1_wavespeeds(Ul[0], Ul + 1, c, d, &a, &b);
+    if (a < sm) sm = a;
+    if (b > sp) sp = b;
+    orc_m1_wavespeeds(Ur[0], Ur + 1, c, d, &a, &b);
+    if (a < sm) sm = a;
+    if (b > sp) sp = b;
+    orc_hll_flux(Ul, gl, Ur, gr, sm, sp, out);
+}
+
+void orc_transport_hll(int nx, int ny, int nz, const double *N, const double *Fx, const double *Fy,
+                       const double *Fz, double c, double dx, double dt,
+                       double *N1, double *Fx1, double *Fy1, double *Fz1) {
+    const long sx = 1, sy = nx, sz = (long)nx * ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; k++)
+        for (int j = 0; j < ny; j++)
+            for (int i = 0; i < nx; i++) {
+                long id = i * sx + j * sy + k * sz;
+                double U[4] = {N[id], Fx[id], Fy[id], Fz[id]};
+                double Un[4] = {U[0], U[1], U[2], U[3]};
+                for (int d = 0; d < 3; d++) {
+                    long ip, im;
+                    if (d == 0) { ip = wrap(i + 1, nx) * sx + j * sy + k * sz; im = wrap(i - 1, nx) * sx + j * sy + k * sz; }
+                    else if (d == 1) { ip = i * sx + wrap(j + 1, ny) * sy + k * sz; im = i * sx + wrap(j - 1, ny) * sy + k * sz; }
+                    else { ip = i * sx + j * sy + wrap(k + 1, nz) * sz; im = i * sx + j * sy + wrap(k - 1, nz) * sz; }
+                    double Up[4] = {N[ip], Fx[ip], Fy[ip], Fz[ip]};
+                    double Um[4] = {N[im], Fx[im], Fy[im], Fz[im]};
+                    double f_hi[4], f_lo[4];
+                    hll_face(d, U, Up, c, f_hi);                                 /* i+1/2 */
+                    hll_face(d, Um, U, c, f_lo);                                 /* i-1/2 */
+                    for (int v = 0; v < 4; v++) Un[v] -= dt / dx * (f_hi[v] - f_lo[v]);   /* Eq.A2 */
                 }
                 N1[id] = Un[0]; Fx1[id] = Un[1]; Fy1[id] = Un[2]; Fz1[id] = Un[3];
             }
@@ -371,7 +451,8 @@ int orc_step(int nx, int ny, int nz, double *N, double *Fx, double *Fy, double *
     if (!buf) return -1;
     double *N1 = buf, *Fx1 = buf + ncell, *Fy1 = buf + 2 * ncell, *Fz1 = buf + 3 * ncell;
     for (int s = 0; s < n_steps; s++) {
-        orc_transport(nx, ny, nz, N, Fx, Fy, Fz, p->c, p->dx, dt, N1, Fx1, Fy1, Fz1);
+        if (p->flux == 1) orc_transport_hll(nx, ny, nz, N, Fx, Fy, Fz, p->c, p->dx, dt, N1, Fx1, Fy1, Fz1);
+        else orc_transport(nx, ny, nz, N, Fx, Fy, Fz, p->c, p->dx, dt, N1, Fx1, Fy1, Fz1);
         memcpy(N, N1, sizeof(double) * ncell);
         memcpy(Fx, Fx1, sizeof(double) * ncell);
         memcpy(Fy, Fy1, sizeof(double) * ncell);

@@ -34,7 +34,7 @@ class Params(C.Structure):
                 ("clump_b", C.c_double), ("redshift", C.c_double), ("eps_sub", C.c_double),
                 ("nH_mean", C.c_double), ("clump_i_a", C.c_double), ("clump_i_b", C.c_double),
                 ("recomb_case", C.c_int), ("cooling", C.c_int),
-                ("coll_ion", C.c_int), ("clump_model", C.c_int), ("max_sub", C.c_int)]
+                ("coll_ion", C.c_int), ("clump_model", C.c_int), ("max_sub", C.c_int), ("flux", C.c_int)]
 
 
 class Rates(C.Structure):
@@ -55,6 +55,10 @@ def lib():
         L.orc_chi.argtypes = [C.c_double]
         L.orc_closure.argtypes = [C.c_double, _dp, C.c_double, _dp]
         L.orc_transport.argtypes = [C.c_int] * 3 + [_dp] * 4 + [C.c_double] * 3 + [_dp] * 4
+        L.orc_transport_hll.argtypes = [C.c_int] * 3 + [_dp] * 4 + [C.c_double] * 3 + [_dp] * 4
+        L.orc_m1_wavespeeds.argtypes = [C.c_double, _dp, C.c_double, C.c_int, _dp, _dp]
+        L.orc_flux_fn.argtypes = [C.c_int, C.c_double, _dp, C.c_double, _dp]
+        L.orc_hll_flux.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, _dp]
         L.orc_inject.argtypes = [C.c_int] * 3 + [_dp, C.c_long, _dp, _dp, C.c_double, C.c_double]
         L.orc_rates.argtypes = [C.c_double, C.POINTER(Rates)]
         L.orc_clumping.restype = C.c_double
@@ -96,7 +100,7 @@ def make_params(params: Dict[str, float], dx: float, nH_mean: float = 1.0) -> Pa
                   clump_i_a=params.get("clump_i_a", 0.0), clump_i_b=params.get("clump_i_b", 0.0),
                   recomb_case=int(params.get("recomb_case", 1)), cooling=int(params.get("cooling", 1)),
                   coll_ion=int(params.get("coll_ion", 1)), clump_model=int(params.get("clump_model", 0)),
-                  max_sub=int(params.get("max_sub", 1 << 14) or (1 << 14)))
+                  max_sub=int(params.get("max_sub", 1 << 14) or (1 << 14)), flux=int(params.get("flux", 0)))
 
 
 def set_threads(n: int) -> None:
@@ -125,6 +129,38 @@ def transport(N, Fx, Fy, Fz, c: float, dx: float, dt: float):
     o = [np.empty_like(a[0]) for _ in range(4)]
     lib().orc_transport(nx, ny, nz, *[_p(v) for v in a], c, dx, dt, *[_p(v) for v in o])
     return tuple(o)
+
+
+def transport_hll(N, Fx, Fy, Fz, c: float, dx: float, dt: float):
+    """One transport step with the HLL intercell flux on [nz,ny,nx] float64 arrays."""
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (N, Fx, Fy, Fz)]
+    nz, ny, nx = a[0].shape
+    o = [np.empty_like(a[0]) for _ in range(4)]
+    lib().orc_transport_hll(nx, ny, nz, *[_p(v) for v in a], c, dx, dt, *[_p(v) for v in o])
+    return tuple(o)
+
+
+def m1_wavespeeds(N: float, F, c: float, d: int):
+    """(lmin, lmax) of the M1 flux Jacobian in direction d (closed form)."""
+    Fa = np.ascontiguousarray(F, dtype=np.float64)
+    lo, hi = C.c_double(), C.c_double()
+    lib().orc_m1_wavespeeds(float(N), _p(Fa), float(c), int(d), C.byref(lo), C.byref(hi))
+    return lo.value, hi.value
+
+
+def flux_fn(d: int, N: float, F, c: float) -> np.ndarray:
+    """Physical flux (F_d, c^2 P_dx, c^2 P_dy, c^2 P_dz) of the 4 conserved variables through a face normal to d."""
+    Fa = np.ascontiguousarray(F, dtype=np.float64)
+    out = np.zeros(4)
+    lib().orc_flux_fn(int(d), float(N), _p(Fa), float(c), _p(out))
+    return out
+
+
+def hll_flux(Ul, gl, Ur, gr, sm: float, sp: float) -> np.ndarray:
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (Ul, gl, Ur, gr)]
+    out = np.zeros(4)
+    lib().orc_hll_flux(*[_p(v) for v in a], float(sm), float(sp), _p(out))
+    return out
 
 
 def inject(N: np.ndarray, pos, rate, dt: float, dx: float) -> None:
