@@ -63,6 +63,9 @@ typedef struct {
     double clump_i_a, clump_i_b; /* photon-atom cross clumping C_I of Eq.15 ("C_I ~ n_H^0.2"):
                             C_I = max(1, a * n_H^b) multiplies the photo-ionisation rate and the absorption;
                             a <= 0 => C_I = 1 (the variant the paper also ran, L269-271) */
+    int flux;            /* intercell flux ("HLL or the simpler Lax-Friedrich scheme"): 0 = Lax-Friedrichs at
+                            speed c (the one the paper used; the product kernel); 1 = HLL with the M1 wave speeds (a
+                            one-thread-per-cell kernel: correct, not tuned; undivided grids only) */
 } aton_params_t;
 
 /* Global diagnostics (PAPER.md:L149 volume-weighted x, L303-305 mass-weighted, Eq.15 Gamma = c sigma_n N). */
@@ -167,12 +170,40 @@ int aton_halo_unpack(aton_t *ctx, const float *recv_lo, const float *recv_hi);
  * a slab must be given the GLOBAL mean (all-reduced by the caller) before aton_set_fields or aton_step. */
 int aton_set_mean_density(aton_t *ctx, double nH_mean);
 
-/* Raw sums of the context's own cells, to be combined across slabs (sum entries 0-10, max 11-12, min 13):
+/* Raw sums of the context's own cells, to be combined across slabs (entries 0-10 and 14 add, 11-12 take the max, 13 the min):
  * [0] cells [1] sum x [2] sum n_H x [3] sum n_H [4] sum N [5] sum n_H N [6] sum T [7] cells with x >= 0.5
- * [8] non-finite cells [9] sub-cycles [10] cells redone by the fix-up [11] max f [12] max sub-cycles [13] min N.
- * n must be ATON_NSUMS.  Synchronises. */
-#define ATON_NSUMS 14
+ * [8] non-finite cells [9] sub-cycles [10] cells redone outside the fast path [11] max f [12] max sub-cycles [13] min N
+ * [14] cells redone in fp64.  n must be ATON_NSUMS.  Synchronises. */
+#define ATON_NSUMS 15
 int aton_reduce_sums(aton_t *ctx, double *sums, int n);
+
+/* The diagnostics of aton_reduce formed from raw sums that the caller has combined across slabs (all the arithmetic of
+ * the means -- <x>_V, <x>_M, Gamma = c sigma_n N, photons = sum N dx^3 -- stays in the library).  No device work. */
+int aton_diag_from_sums(aton_t *ctx, const double *sums, int n, aton_diag_t *out);
+
+/* <n_H> of the linear clumping law from combined raw sums: aton_set_mean_density(ctx, sums[3] / sums[0]). */
+int aton_set_mean_from_sums(aton_t *ctx, const double *sums, int n);
+
+/* ---- the same slabs with the exchange inside the library (one call per run of steps, exchange overlapped) ----
+ *
+ * aton_comm_unique_id: rank 0 obtains an id (ATON_COMM_ID_BYTES bytes, an ncclUniqueId) and hands it to every rank by
+ * whatever means the caller has.  aton_comm_init(ctx, id, nbytes, rank, world) then creates the library's own NCCL
+ * communicator over the `world` slab contexts (rank r owns the r-th slab in z order; collective: every rank calls it),
+ * a second CUDA stream and the events of the overlap.  id == NULL is allowed for world == 1 (the slab spans the whole
+ * grid and wraps onto itself by device copies; no NCCL needed).  libnccl.so.2 is looked up at run time.
+ *
+ * aton_step_slab(ctx, dt, n_steps): n steps; each step computes the slab's two boundary planes first, sends them
+ * (ncclSend / ncclRecv straight out of / into the field arrays: no pack / unpack, no host staging -- the paper's
+ * exchange costs 10-15 % of a step) on the second stream while the interior planes are computed, and the
+ * next step's boundary kernels wait for the arrival.  Collective; asynchronous on the context's streams; bit-identical
+ * to the undivided run.  aton_reduce_global all-gathers the raw sums and returns the diagnostics of the WHOLE box;
+ * aton_sync_mean_density makes <n_H> of the linear clumping law the global mean (call it once after aton_set_fields). */
+#define ATON_COMM_ID_BYTES 128
+int aton_comm_unique_id(unsigned char *id, int nbytes);
+int aton_comm_init(aton_t *ctx, const unsigned char *id, int nbytes, int rank, int world);
+int aton_step_slab(aton_t *ctx, double dt, int n_steps);
+int aton_reduce_global(aton_t *ctx, aton_diag_t *out);
+int aton_sync_mean_density(aton_t *ctx);
 
 void aton_free(aton_t *ctx);
 

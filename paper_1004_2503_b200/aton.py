@@ -20,8 +20,10 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt", "aton_step",
            "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_set_timing",
            "aton_kernel_time", "aton_fixup_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
-           "aton_reduce_sums", "aton_free", "aton_last_error")
-NSUMS = 14
+           "aton_reduce_sums", "aton_diag_from_sums", "aton_set_mean_from_sums", "aton_comm_unique_id", "aton_comm_init",
+           "aton_step_slab", "aton_reduce_global", "aton_sync_mean_density", "aton_free", "aton_last_error")
+COMM_ID_BYTES = 128
+NSUMS = 15
 
 
 class Grid(C.Structure):
@@ -37,7 +39,7 @@ class Params(C.Structure):
                 ("e_photon_eV", C.c_double), ("recomb_case", C.c_int), ("cooling", C.c_int),
                 ("coll_ion", C.c_int), ("clump_model", C.c_int), ("clump_a", C.c_double),
                 ("clump_b", C.c_double), ("redshift", C.c_double), ("eps_sub", C.c_double),
-                ("max_sub", C.c_int), ("clump_i_a", C.c_double), ("clump_i_b", C.c_double)]
+                ("max_sub", C.c_int), ("clump_i_a", C.c_double), ("clump_i_b", C.c_double), ("flux", C.c_int)]
 
 
 class Diag(C.Structure):
@@ -103,6 +105,20 @@ def load_library(path: Optional[str] = None):
     L.aton_set_mean_density.argtypes = [vp, C.c_double]
     L.aton_reduce_sums.restype = C.c_int
     L.aton_reduce_sums.argtypes = [vp, C.POINTER(C.c_double), C.c_int]
+    L.aton_diag_from_sums.restype = C.c_int
+    L.aton_diag_from_sums.argtypes = [vp, C.POINTER(C.c_double), C.c_int, C.POINTER(Diag)]
+    L.aton_set_mean_from_sums.restype = C.c_int
+    L.aton_set_mean_from_sums.argtypes = [vp, C.POINTER(C.c_double), C.c_int]
+    L.aton_comm_unique_id.restype = C.c_int
+    L.aton_comm_unique_id.argtypes = [C.c_char_p, C.c_int]
+    L.aton_comm_init.restype = C.c_int
+    L.aton_comm_init.argtypes = [vp, C.c_char_p, C.c_int, C.c_int, C.c_int]
+    L.aton_step_slab.restype = C.c_int
+    L.aton_step_slab.argtypes = [vp, C.c_double, C.c_int]
+    L.aton_reduce_global.restype = C.c_int
+    L.aton_reduce_global.argtypes = [vp, C.POINTER(Diag)]
+    L.aton_sync_mean_density.restype = C.c_int
+    L.aton_sync_mean_density.argtypes = [vp]
     L.aton_free.restype = None
     L.aton_free.argtypes = [vp]
     L.aton_last_error.restype = C.c_char_p
@@ -226,6 +242,32 @@ class Aton:
         self._check(self._L.aton_reduce_sums(self._h, buf, NSUMS))
         return list(buf)
 
+    def diag_from_sums(self, sums) -> Dict[str, float]:
+        """aton_diag_t formed by the library from raw sums the caller combined across slabs."""
+        buf = (C.c_double * NSUMS)(*sums)
+        d = Diag()
+        self._check(self._L.aton_diag_from_sums(self._h, buf, NSUMS, C.byref(d)))
+        return {k: getattr(d, k) for k, _ in Diag._fields_}
+
+    def set_mean_from_sums(self, sums):
+        buf = (C.c_double * NSUMS)(*sums)
+        self._check(self._L.aton_set_mean_from_sums(self._h, buf, NSUMS))
+
+    def comm_init(self, comm_id: Optional[bytes], rank: int, world: int):
+        """aton_comm_init: `comm_id` = the bytes of comm_unique_id() from rank 0 (None only for world == 1)."""
+        self._check(self._L.aton_comm_init(self._h, comm_id, COMM_ID_BYTES if comm_id is not None else 0, rank, world))
+
+    def step_slab(self, dt: float, n_steps: int = 1):
+        self._check(self._L.aton_step_slab(self._h, float(dt), int(n_steps)))
+
+    def reduce_global(self) -> Dict[str, float]:
+        d = Diag()
+        self._check(self._L.aton_reduce_global(self._h, C.byref(d)))
+        return {k: getattr(d, k) for k, _ in Diag._fields_}
+
+    def sync_mean_density(self):
+        self._check(self._L.aton_sync_mean_density(self._h))
+
     def set_timing(self, on: bool):
         self._check(self._L.aton_set_timing(self._h, int(bool(on))))
 
@@ -243,6 +285,15 @@ class Aton:
 
     def launch_count(self) -> int:
         return int(self._L.aton_launch_count(self._h))
+
+
+def comm_unique_id() -> bytes:
+    """An ncclUniqueId for aton_comm_init, as bytes (rank 0 calls this and distributes the result)."""
+    buf = C.create_string_buffer(COMM_ID_BYTES)
+    rc = load_library().aton_comm_unique_id(buf, COMM_ID_BYTES)
+    if rc != OK:
+        raise AtonError(rc, load_library().aton_last_error(None).decode())
+    return buf.raw
 
 
 def from_workload(w, stream=None, device="cuda") -> Aton:

@@ -18,14 +18,15 @@ def sources():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/aton_api.cu (which includes every kernel header) into libaton.so."""
+    """Compile every csrc/*.cu (aton_api.cu holds the step kernels' instantiations) into libaton.so."""
     newest = max(os.path.getmtime(s) for s in sources())
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".{os.getpid()}.tmp"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", tmp, os.path.join(CSRC, "aton_api.cu")]
+    units = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    cmd = [nvcc] + NVCC_FLAGS + ["--threads", str(len(units))] + (["-Xptxas", "-v"] if verbose else []) + \
+          ["-o", tmp] + units + ["-ldl"]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

@@ -2,96 +2,18 @@
 // loop and the diagnostics.  The host only drives; every step of the path runs in
 // the kernels of aton_step_v4.cuh (product), aton_fixup.cuh, aton_step_fused.cuh / aton_step_ref.cuh
 // (fallback / cross-check) and aton_reduce.cuh.
-#include <cuda_runtime.h>
-
-#include <algorithm>
-#include <cmath>
-#include <cstdarg>
-#include <cstdio>
-#include <cstdlib>
-#include <cstring>
-#include <new>
-#include <vector>
-
-#include "../../include/aton.h"
-#include "aton_physics.cuh"
+#include "aton_ctx.cuh"
 #include "aton_reduce.cuh"
-#include "aton_step_ref.cuh"
 #include "aton_step_fused.cuh"
-#include "aton_fixup.cuh"
 #include "aton_step_v4.cuh"
 
 using namespace aton;
 
-namespace {
-
-constexpr double K_BOLTZ = 1.380649e-16, EV_ERG = 1.602176634e-12, E0_EV = 13.6;
-constexpr int REDUCE_BLOCKS = 148 * 8;
-constexpr int N_STATS = 4;
-
+namespace aton {
 char g_init_error[512] = "";
-
-}  // namespace
-
-struct aton_ctx {
-    Grid g{};
-    size_t ncell = 0;                      // cells this context advances (the slab's own planes)
-    size_t nalloc = 0, plane = 0, off = 0; // allocated cells per array (slab: + 2 ghost planes), nx*ny, first own cell
-    bool slab = false;                     // aton_init_slab: planes [z_begin, z_begin + nz_local) of a global grid
-    int z_begin = 0, nz_local = 0, nz_global = 0;
-    bool mean_set = false;                 // aton_set_mean_density overrides <n_H> of aton_set_fields
-    double dx = 0, c = 0;
-    aton_params_t p{};
-    cudaStream_t stream = nullptr;
-    float *rad[2][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};
-    float *x = nullptr, *T = nullptr, *nH = nullptr;
-    int cur = 0;
-    unsigned *src_mask = nullptr;
-    int *src_cell = nullptr;
-    float *src_rho = nullptr;
-    double *src_rho_d = nullptr;
-    int n_src = 0;
-    int device = 0;                        // the device current at aton_init; every entry point runs there
-    unsigned long long *stats = nullptr;   // device [4]
-    unsigned *defer_mask = nullptr;        // device, 1 bit per cell (variant 2)
-    unsigned *src_bits = nullptr;          // device, 1 bit per cell: the cell holds a source (variant 4)
-    int *stiff_q = nullptr;                // device [stiff_cap]: ids of the cells to redo in fp64 (variant 4)
-    unsigned *stiff_n = nullptr;           // device [2]
-    unsigned stiff_cap = 0;
-    FixArgs *fixargs = nullptr;            // device [2]: what the cold paths of variant 4 read, per ping-pong parity
-    bool fix_dirty = true;                 // fixargs must be rewritten (dt, sources, <n_H> or buffers changed)
-    double fix_dt = -1.0;
-    long long fast_subcycles = 0;          // variant 2: one sub-cycle per cell and step, counted on the host
-    double *partials = nullptr;            // device [REDUCE_BLOCKS+1][R_COUNT]
-    double nH_mean = 1.0;
-    bool have_fields = false;
-    long long steps_done = 0, launches = 0;
-    double time_s = 0;
-    int variant = 4, tile_y = 0, tile_z = 0;
-    bool timing = false;                   // aton_set_timing: CUDA events around the kernels of a step
-    std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch of the dominant step kernel
-    std::vector<cudaEvent_t> ev_fix;       // the same for the second kernel of a step (fp64 redo / mask fix-up)
-    char err[512] = "";
-};
-
-namespace {
-
-int fail(aton_ctx *ctx, int code, const char *fmt, ...) {
-    char *dst = ctx ? ctx->err : g_init_error;
-    va_list ap;
-    va_start(ap, fmt);
-    vsnprintf(dst, 512, fmt, ap);
-    va_end(ap);
-    return code;
 }
 
-#define CU(ctx, call)                                                                         \
-    do {                                                                                      \
-        cudaError_t e_ = (call);                                                              \
-        if (e_ != cudaSuccess)                                                                \
-            return fail(ctx, e_ == cudaErrorMemoryAllocation ? ATON_ENOMEM : ATON_ECUDA,      \
-                        "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
-    } while (0)
+namespace {
 
 int flags_of(const aton_params_t &p) {
     return (p.recomb_case == 0 ? F_CASE_A : 0) | (p.cooling ? F_COOL : 0) | (p.coll_ion ? F_COLL : 0);
@@ -129,6 +51,11 @@ StepConst make_step_const(const aton_ctx *ctx, double dt) {
     s.ci_k0 = p.clump_i_a > 0.0 ? (float)p.clump_i_a : 0.0f;
     s.ci_k1 = (float)p.clump_i_b;
     s.inj_scale = 0.0f;
+    // when the fp32 sub-cycling hands a cell to the fp64 path (chemistry<.., BAIL>; thresholds measured against the
+    // 1-step bar at 256^3 / 512^3 / 1024^3: profiles/r02_b_fixup.md)
+    s.stiff_kappa = 1.0f / 64.0f;
+    s.stiff_sens = 1.0f;
+    s.stiff_nsub = 1 << 30;
     return s;
 }
 
@@ -174,23 +101,11 @@ FieldsIO make_io(const aton_ctx *ctx, int cur) {
     f.defer_mask = ctx->defer_mask;
     f.src_bits = ctx->src_bits;
     f.stiff_q = ctx->stiff_q; f.stiff_n = ctx->stiff_n; f.stiff_cap = ctx->stiff_cap;
+    f.fix_inject = (ctx->variant == 4 && v4_pick_wxq(ctx->g, ctx->tile_y) != 0) ? 1 : 0;
     return f;
 }
 
 __global__ void write_fixargs_kernel(FixArgs a0, FixArgs a1, FixArgs *dst) { dst[0] = a0; dst[1] = a1; }
-
-// variant 4's cold paths (v4_fix_batch, step_stiff_kernel) read their arguments from global memory; rewrite them
-// (stream-ordered, no host synchronisation) only when something they hold has changed
-cudaError_t sync_fixargs(aton_ctx *ctx, const StepConst &sc, const StepConstD &scd, double dt) {
-    if (!ctx->fix_dirty && ctx->fix_dt == dt) return cudaSuccess;
-    FixArgs a[2];
-    for (int cur = 0; cur < 2; cur++) { a[cur].f = make_io(ctx, cur); a[cur].c = sc; a[cur].cd = scd; }
-    write_fixargs_kernel<<<1, 1, 0, ctx->stream>>>(a[0], a[1], ctx->fixargs);
-    ctx->launches++;
-    ctx->fix_dirty = false;
-    ctx->fix_dt = dt;
-    return cudaGetLastError();
-}
 
 // aton_set_timing: an event right before / after the dominant kernel of a step
 void time_mark(aton_ctx *ctx) {
@@ -210,7 +125,17 @@ void fix_mark(aton_ctx *ctx) {
 }
 
 template <int FLAGS>
-cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc, const StepConstD &scd) {
+cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
+    const StepConst &sc = ctx->sc;
+    const StepConstD &scd = ctx->scd;
+    if (ctx->p.flux == 1) {        // HLL intercell flux: one-thread-per-cell kernel, whatever the variant
+        const int threads = 256;
+        const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
+        time_mark(ctx);
+        step_hll_kernel<FLAGS><<<blocks, threads, 0, ctx->stream>>>(f, ctx->g, sc, scd);
+        time_mark(ctx);
+        return cudaGetLastError();
+    }
     if (ctx->variant == 0) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
@@ -220,48 +145,45 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, const StepConst &sc, co
         return cudaGetLastError();
     }
     // variant 4 needs nx % 32 == 0 and ny % 4 == 0 (or nx % 64 == 0 and ny % 2 == 0); other grids run the variant-2
-    // kernel.  Variant 4 leaves the source cells and the sub-cycling cells to its own warp-level redo + the fp64
-    // kernel; variant 2 injects in the step kernel and flags the sub-cycling cells for step_fixup_kernel.
+    // kernel.  Both flag the cells that sub-cycle for step_fixup_kernel; variant 4 also flags its source cells (the
+    // fix-up injects), variant 2 injects in the step kernel.
     const int wxq4 = ctx->variant == 4 ? v4_pick_wxq(ctx->g, ctx->tile_y) : 0;
     if (ctx->slab && !wxq4) return cudaErrorNotSupported;    // checked with a message in aton_step
-    ctx->fast_subcycles += (long long)ctx->ncell;
+    ctx->fast_subcycles += (long long)ctx->plane * (ze - zb);
     cudaError_t e;
-    if (wxq4) {
-        time_mark(ctx);
-        e = launch_step_v4<FLAGS>(f, ctx->g, sc, ctx->fixargs + ctx->cur, wxq4, ctx->tile_z, ctx->stream, ctx->slab ? 1 : 0,
-                                  ctx->slab ? ctx->nz_local + 1 : ctx->g.nz);
-        time_mark(ctx);
-        if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;   // without cooling nothing sub-cycles: no cell can be stiff
-        ctx->launches++;
-        fix_mark(ctx);
-        e = launch_step_stiff<FLAGS>(ctx->fixargs + ctx->cur, ctx->stream);
-        fix_mark(ctx);
-        return e;
-    }
     time_mark(ctx);
-    e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0, ctx->variant == 2 ? ctx->tile_z : 0,
-                                 ctx->stream);
+    if (wxq4)
+        e = launch_step_v4<FLAGS>(f, ctx->g, sc, wxq4, ctx->tile_z, ctx->stream, zb, ze);
+    else
+        e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0, ctx->variant == 2 ? ctx->tile_z : 0,
+                                     ctx->stream);
     time_mark(ctx);
-    if (e != cudaSuccess || !(FLAGS & F_COOL)) return e;
-    ctx->launches++;
+    // the second half of a step: cells that sub-cycle (cooling on) and, for variant 4, the source cells
+    if (e != cudaSuccess || !((FLAGS & F_COOL) || (wxq4 && ctx->n_src > 0))) return e;
+    (void)scd;
     fix_mark(ctx);
-    e = launch_step_fixup<FLAGS>(f, ctx->g, sc, scd, ctx->stream);
+    ctx->launches++;
+    e = launch_step_fixup<FLAGS>(ctx->fixargs + ctx->cur, (long)ctx->plane * zb, (long)ctx->plane * ze, ctx->stream);
+    if (e == cudaSuccess && (FLAGS & F_COOL)) {       // without cooling nothing sub-cycles: no cell can be stiff
+        ctx->launches++;
+        e = launch_step_stiff<FLAGS>(ctx->fixargs + ctx->cur, ctx->stream);
+    }
     fix_mark(ctx);
     return e;
 }
 
-cudaError_t launch_step(aton_ctx *ctx, const StepConst &sc, const StepConstD &scd) {
+cudaError_t launch_step(aton_ctx *ctx, int zb, int ze) {
     const FieldsIO f = make_io(ctx, ctx->cur);
     ctx->launches++;
     switch (flags_of(ctx->p)) {
-        case 0: return launch_one<0>(ctx, f, sc, scd);
-        case 1: return launch_one<1>(ctx, f, sc, scd);
-        case 2: return launch_one<2>(ctx, f, sc, scd);
-        case 3: return launch_one<3>(ctx, f, sc, scd);
-        case 4: return launch_one<4>(ctx, f, sc, scd);
-        case 5: return launch_one<5>(ctx, f, sc, scd);
-        case 6: return launch_one<6>(ctx, f, sc, scd);
-        default: return launch_one<7>(ctx, f, sc, scd);
+        case 0: return launch_one<0>(ctx, f, zb, ze);
+        case 1: return launch_one<1>(ctx, f, zb, ze);
+        case 2: return launch_one<2>(ctx, f, zb, ze);
+        case 3: return launch_one<3>(ctx, f, zb, ze);
+        case 4: return launch_one<4>(ctx, f, zb, ze);
+        case 5: return launch_one<5>(ctx, f, zb, ze);
+        case 6: return launch_one<6>(ctx, f, zb, ze);
+        default: return launch_one<7>(ctx, f, zb, ze);
     }
 }
 
@@ -272,6 +194,65 @@ int scale_into(aton_ctx *ctx, const float *in, float *out, float s) {
     ctx->launches++;
     CU(ctx, cudaGetLastError());
     return ATON_OK;
+}
+
+}  // namespace
+
+namespace aton {
+
+int check_dt(aton_ctx *ctx, double *dt, const char *who) {
+    if (!(*dt > 0.0)) *dt = aton_courant_dt(ctx, 0.8);
+    const double mu = ctx->c * *dt / ctx->dx;
+    if (!(mu <= (1.0 / 3.0) * (1.0 + 1e-12)) || !std::isfinite(mu))
+        return fail(ctx, ATON_EINVAL, "%s: c*dt/dx = %g > 1/3 is unstable for the unsplit 3-D LF scheme", who, mu);
+    return ATON_OK;
+}
+
+// Step constants for dt, and the arguments variant 4's cold paths (v4_fix_drain, step_fixup_kernel, step_stiff_kernel)
+// read from global memory: rewritten (stream-ordered, no host synchronisation) only when something they hold changed.
+cudaError_t prepare_step(aton_ctx *ctx, double dt) {
+    if (!ctx->fix_dirty && ctx->fix_dt == dt) return cudaSuccess;
+    ctx->sc = make_step_const(ctx, dt);
+    ctx->scd = make_step_const_d(ctx, dt);
+    FixArgs a[2];
+    for (int cur = 0; cur < 2; cur++) { a[cur].f = make_io(ctx, cur); a[cur].c = ctx->sc; a[cur].cd = ctx->scd; }
+    write_fixargs_kernel<<<1, 1, 0, ctx->stream>>>(a[0], a[1], ctx->fixargs);
+    ctx->launches++;
+    ctx->fix_dirty = false;
+    ctx->fix_dt = dt;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step_planes(aton_ctx *ctx, int zb, int ze) { return launch_step(ctx, zb, ze); }
+
+// raw sums of the context's own cells in the order of aton_reduce_sums (include/aton.h)
+void sums_from_reduce(aton_ctx *ctx, const double *r, const unsigned long long *st, double *sums) {
+    sums[0] = (double)ctx->ncell; sums[1] = r[R_X]; sums[2] = r[R_XM]; sums[3] = r[R_M]; sums[4] = r[R_N];
+    sums[5] = r[R_NM]; sums[6] = r[R_T]; sums[7] = r[R_HALF]; sums[8] = r[R_BAD];
+    sums[9] = (double)((long long)st[0] + ctx->fast_subcycles); sums[10] = (double)st[2];
+    sums[11] = std::sqrt(r[R_F2MAX]); sums[12] = (double)std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
+    sums[13] = r[R_NMIN]; sums[14] = (double)st[3];
+}
+
+// the diagnostics of PAPER.md:L149 / L303-305 / Eq.15 from (possibly all-reduced) raw sums
+void diag_from_sums(const aton_ctx *ctx, const double *s, aton_diag_t *out) {
+    const double n = s[0], cs = ctx->c * ctx->p.sigma_n;
+    out->x_vol = s[1] / n;
+    out->x_mass = s[2] / s[3];
+    out->gamma_vol = cs * s[4] / n;
+    out->gamma_mass = cs * s[5] / s[3];
+    out->photons_total = s[4] * ctx->dx * ctx->dx * ctx->dx;
+    out->T_vol = s[6] / n;
+    out->f_max = s[11];
+    out->N_min = s[13];
+    out->frac_x_half = s[7] / n;
+    out->n_nonfinite = (long long)s[8];
+    out->subcycles_total = (long long)s[9];
+    out->subcycles_max = (long long)s[12];
+    out->cells_subcycled = (long long)s[10];
+    out->cells_fp64 = (long long)s[14];
+    out->steps_done = ctx->steps_done;
+    out->time_s = ctx->time_s;
 }
 
 // run the two-pass reduction; host_out[R_COUNT]
@@ -294,7 +275,7 @@ int run_reduce(aton_ctx *ctx, bool full, double *host_out) {
     return ATON_OK;
 }
 
-}  // namespace
+}  // namespace aton
 
 extern "C" {
 
@@ -317,8 +298,10 @@ static int init_common(aton_t **out, const aton_grid_t *grid, const aton_box_t *
     if (!(params->sigma_n > 0.0) || !(params->sigma_e > 0.0) || !(params->e_photon_eV > 0.0))
         return fail(nullptr, ATON_EINVAL, "aton_init: sigma_n, sigma_e, e_photon_eV must be > 0");
     if (params->clump_model < 0 || params->clump_model > 2 || params->c_cm_s < 0.0 || params->eps_sub < 0.0 ||
-        params->max_sub < 0)
-        return fail(nullptr, ATON_EINVAL, "aton_init: bad clump_model / c / eps_sub / max_sub");
+        params->max_sub < 0 || params->flux < 0 || params->flux > 1)
+        return fail(nullptr, ATON_EINVAL, "aton_init: bad clump_model / c / eps_sub / max_sub / flux");
+    if (slab && params->flux != 0)
+        return fail(nullptr, ATON_EINVAL, "aton_init_slab: the HLL flux runs on undivided grids only");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -387,6 +370,7 @@ int aton_init_slab(aton_t **out, const aton_grid_t *global_grid, const aton_box_
 void aton_free(aton_t *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    slab_comm_free(ctx);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
     for (int b = 0; b < 2; b++)
@@ -409,6 +393,7 @@ int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if ((variant == 2 && !fused_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
+    ctx->fix_dirty = true;
     return ATON_OK;
 }
 
@@ -457,6 +442,7 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
     const size_t bytes = ctx->ncell * sizeof(float);
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     ctx->have_fields = false;
+    ctx->halo_valid = false;
     ctx->cur = 0;
     const size_t o = ctx->off;             // a slab's own planes start one (ghost) plane in
     CU(ctx, cudaMemcpyAsync(ctx->nH + o, nH, bytes, kind, ctx->stream));
@@ -576,23 +562,19 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     if (!ctx) return ATON_EINVAL;
     if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_step: call aton_set_fields first");
     if (n_steps < 0) return fail(ctx, ATON_EINVAL, "aton_step: n_steps < 0");
-    if (!(dt > 0.0)) dt = aton_courant_dt(ctx, 0.8);
-    const double mu = ctx->c * dt / ctx->dx;
-    if (!(mu <= (1.0 / 3.0) * (1.0 + 1e-12)) || !std::isfinite(mu))
-        return fail(ctx, ATON_EINVAL, "aton_step: c*dt/dx = %g > 1/3 is unstable for the unsplit 3-D LF scheme", mu);
+    if (int rc = check_dt(ctx, &dt, "aton_step")) return rc;
     if (ctx->slab && ctx->variant != 4)
         return fail(ctx, ATON_ESTATE, "aton_step: a slab context runs kernel variant 4 only");
     if (ctx->slab && n_steps > 1)
-        return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first)");
-    const StepConst sc = make_step_const(ctx, dt);
-    const StepConstD scd = make_step_const_d(ctx, dt);
-    if (n_steps > 0) CU(ctx, sync_fixargs(ctx, sc, scd, dt));
+        return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first, or use aton_step_slab)");
+    if (n_steps > 0) CU(ctx, prepare_step(ctx, dt));
     for (int s = 0; s < n_steps; s++) {
-        CU(ctx, launch_step(ctx, sc, scd));
+        CU(ctx, launch_step_planes(ctx, ctx->slab ? 1 : 0, ctx->slab ? ctx->nz_local + 1 : ctx->g.nz));
         ctx->cur = 1 - ctx->cur;
         ctx->steps_done++;
         ctx->time_s += dt;
     }
+    ctx->halo_valid = false;
     return ATON_OK;
 }
 
@@ -644,12 +626,23 @@ int aton_reduce_sums(aton_t *ctx, double *sums, int n) {
     unsigned long long st[N_STATS];
     CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
     CU(ctx, cudaStreamSynchronize(ctx->stream));
-    sums[0] = (double)ctx->ncell; sums[1] = r[R_X]; sums[2] = r[R_XM]; sums[3] = r[R_M]; sums[4] = r[R_N];
-    sums[5] = r[R_NM]; sums[6] = r[R_T]; sums[7] = r[R_HALF]; sums[8] = r[R_BAD];
-    sums[9] = (double)((long long)st[0] + ctx->fast_subcycles); sums[10] = (double)st[2];
-    sums[11] = std::sqrt(r[R_F2MAX]); sums[12] = (double)std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
-    sums[13] = r[R_NMIN];
+    sums_from_reduce(ctx, r, st, sums);
     return ATON_OK;
+}
+
+int aton_diag_from_sums(aton_t *ctx, const double *sums, int n, aton_diag_t *out) {
+    if (!ctx || !sums || !out) return ATON_EINVAL;
+    if (n != ATON_NSUMS) return fail(ctx, ATON_EINVAL, "aton_diag_from_sums: n must be ATON_NSUMS (%d)", ATON_NSUMS);
+    if (!(sums[0] > 0.0) || !(sums[3] > 0.0)) return fail(ctx, ATON_EINVAL, "aton_diag_from_sums: no cells / no mass in the sums");
+    diag_from_sums(ctx, sums, out);
+    return ATON_OK;
+}
+
+int aton_set_mean_from_sums(aton_t *ctx, const double *sums, int n) {
+    if (!ctx || !sums) return ATON_EINVAL;
+    if (n != ATON_NSUMS) return fail(ctx, ATON_EINVAL, "aton_set_mean_from_sums: n must be ATON_NSUMS (%d)", ATON_NSUMS);
+    if (!(sums[0] > 0.0)) return fail(ctx, ATON_EINVAL, "aton_set_mean_from_sums: no cells in the sums");
+    return aton_set_mean_density(ctx, sums[3] / sums[0]);
 }
 
 int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float *Fx, float *Fy, float *Fz,
@@ -683,30 +676,10 @@ int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float 
 
 int aton_reduce(aton_t *ctx, aton_diag_t *out) {
     if (!ctx || !out) return ATON_EINVAL;
-    if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_reduce: no fields set");
-    double r[R_COUNT];
-    int rc = run_reduce(ctx, true, r);
+    double sums[ATON_NSUMS];
+    int rc = aton_reduce_sums(ctx, sums, ATON_NSUMS);
     if (rc) return rc;
-    unsigned long long st[N_STATS];
-    CU(ctx, cudaMemcpyAsync(st, ctx->stats, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
-    CU(ctx, cudaStreamSynchronize(ctx->stream));
-    const double n = (double)ctx->ncell, cs = ctx->c * ctx->p.sigma_n;
-    out->x_vol = r[R_X] / n;
-    out->x_mass = r[R_XM] / r[R_M];
-    out->gamma_vol = cs * r[R_N] / n;
-    out->gamma_mass = cs * r[R_NM] / r[R_M];
-    out->photons_total = r[R_N] * ctx->dx * ctx->dx * ctx->dx;
-    out->T_vol = r[R_T] / n;
-    out->f_max = std::sqrt(r[R_F2MAX]);
-    out->N_min = r[R_NMIN];
-    out->frac_x_half = r[R_HALF] / n;
-    out->n_nonfinite = (long long)r[R_BAD];
-    out->subcycles_total = (long long)st[0] + ctx->fast_subcycles;
-    out->subcycles_max = std::max((long long)st[1], ctx->fast_subcycles > 0 ? 1LL : 0LL);
-    out->cells_subcycled = (long long)st[2];
-    out->cells_fp64 = (long long)st[3];
-    out->steps_done = ctx->steps_done;
-    out->time_s = ctx->time_s;
+    diag_from_sums(ctx, sums, out);
     return ATON_OK;
 }
 

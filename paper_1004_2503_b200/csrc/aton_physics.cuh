@@ -35,6 +35,9 @@ struct StepConst {        // per aton_step call, host-computed in fp64, passed b
     float clump_k0, clump_k1;  // model 1: C = max(1, k0 + k1*nH); model 2: C = max(1, k0 * nH^k1)
     float ci_k0, ci_k1;   // C_I = max(1, k0 * nH^k1) on photo-ionisation and absorption; k0 <= 0: off (C_I = 1)
     float inj_scale;      // dt / dx^3 folded into the per-source density rate
+    float stiff_kappa;    // BAIL: hand a cell to the fp64 path when |H - Lambda| < kappa (H + |Lambda|) limits a sub-step,
+    float stiff_sens;     // ... when the attenuation's sensitivity to the sub-step partition, sum A y'/(1 + A y'), exceeds this
+    int stiff_nsub;       // ... or when it needs more than this many sub-cycles
 };
 
 // ---------------------------------------------------------------- MUFU wrappers
@@ -153,7 +156,6 @@ __device__ __forceinline__ float clumping_i(float nH, const StepConst &c) {
 // BAIL: give up (return -1, in/out values then meaningless) as soon as a sub-step is limited by the 10 % rule while
 // heating and cooling cancel to better than STIFF_KAPPA: the sub-step eps E/|H - Lambda| is then ill-conditioned
 // (the fp32 rate fits carry ~3e-6) and the caller redoes the cell with chemistry_f64 (aton_physics_f64.cuh).
-constexpr float STIFF_KAPPA = 1.0f / 64.0f;
 
 template <int FLAGS, bool BAIL = false>
 __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &gz, float &x, float &T,
@@ -168,10 +170,12 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
     float t_left = c.dt;
     int nsub = 0;
     float att_tot = 1.0f;
+    float y = 1.0f - x;          // carried: y' = y - delta keeps the neutral fraction's own digits (never 1 - x', H1)
+    float sens = 0.0f;
     while (t_left > 0.0f && nsub < c.max_sub) {
+        if (BAIL && nsub >= c.stiff_nsub) return -1;
         Rates r;
         rates<FLAGS>(T, c, r);
-        const float y = 1.0f - x;
         const float ne = x * nH;
         const float theta = (1.0f + x) * T;
         float dts = t_left;
@@ -181,7 +185,7 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
             const float heat = y * N * heat_rate;
             float ed = fabsf(heat - lamK);
             if (ed * t_left > c.eps_sub * theta) {
-                if (BAIL && ed < STIFF_KAPPA * (heat + fabsf(lamK))) return -1;
+                if (BAIL && ed < c.stiff_kappa * (heat + fabsf(lamK))) return -1;
                 dts = c.eps_sub * theta / ed;
             }
         }
@@ -204,6 +208,12 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
         const float xn = fminf(fmaxf(x + delta, 0.0f), 1.0f);
         const float yn = fmaxf(y - delta, 0.0f);
         const float att = f_rcp(fmaf(A, yn, 1.0f));
+        if (BAIL) {
+            // N' = N prod_k 1/(1 + A_k y'_k): a relative error e_k of the k-th sub-step length moves ln N' by
+            // e_k A y'/(1 + A y'), and the fp32 heating estimate carries e_k ~ 4e-6
+            sens += 1.0f - att;
+            if (sens > c.stiff_sens && dts < t_left) return -1;
+        }
         const float Pa = P * att;
         N = nH * Pa;
         att_tot *= att;
@@ -219,6 +229,7 @@ __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &
             T = fmaxf(thn * f_rcp(1.0f + xn), 1.0f);
         }
         x = xn;
+        y = yn;
         t_left -= dts;
         ++nsub;
     }

@@ -19,8 +19,9 @@
 //    no source lookups -- the scheduler interleaves the chemistry's MUFU chains with the transport FMAs;
 //  * per-cell source flags come from a 1-bit-per-cell mask: a source cell is treated like a cell that
 //    needs sub-cycling (chemistry result discarded, flagged); the fix-up kernel injects and sub-cycles.
-//  * cells that need sub-cycling (and the source cells) are redone by the warp itself, 32 at a time, from a
-//    warp-private shared-memory queue (aton_fixup.cuh): their lines are still in L2 when the results land.
+//  * cells that need sub-cycling (and the source cells) keep their transported values, are flagged in a 1-bit-per-cell
+//    mask and are redone by step_fixup_kernel (aton_fixup.cuh).  Redoing them inside this kernel (a warp-private queue
+//    drained 32 cells at a time) was built and measured in round 2: slower in every state (profiles/r02_b_fixup.md).
 #pragma once
 #include <type_traits>
 
@@ -32,6 +33,9 @@ namespace aton {
 #ifndef ATON_V4_WARPS
 #define ATON_V4_WARPS 4
 #endif
+#ifndef ATON_V4_YSHFL
+#define ATON_V4_YSHFL 1   // y neighbour terms by warp shuffles (no shared-memory patch, no __syncwarp): A/B in profiles/r02_c_step_v4.md
+#endif
 // WXQ = quads per tile row: 8 -> a 32 x 4 tile (the default), 16 -> 64 x 2
 template <int WXQ>
 struct V4Cfg {
@@ -41,8 +45,11 @@ struct V4Cfg {
     static constexpr int RAW_BUF = 4 * RAW_FIELD;        // [field][slot][RS]
     static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
     static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][WX]
-    static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN + V4_QWORDS;   // + the warp's deferred-cell queue
+    static constexpr int WARP_FLOATS = 2 * RAW_BUF + (ATON_V4_YSHFL ? 0 : 2 * W_SIGN);
     static constexpr int WARPS = ATON_V4_WARPS, THREADS = 32 * WARPS;
+    // 47 104 B per CTA for the 32 x 4 tile: 4 CTAs fit the 196 KB shared-memory carve-out and leave 60 KB of L1 for the
+    // halo re-reads.  768 B more per warp (tried: a queue of deferred cells) falls into the 228 KB carve-out, 28 KB of
+    // L1, and costs 3.4 ms per 1024^3 step (profiles/r02_b_fixup.md).
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * sizeof(float);
 };
 
@@ -90,7 +97,7 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
 #endif
 template <int FLAGS, int WXQ>
 __global__ void __launch_bounds__(V4Cfg<WXQ>::THREADS, ATON_V4_MINB)
-step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int zb, int ze) {
+step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     using C = V4Cfg<WXQ>;
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -98,12 +105,10 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
     const int xt = blockIdx.x * C::WARPS + warp;         // x tile of this warp
     if (xt * C::WX >= g.nx) return;                      // ragged last CTA in x: warps are independent
     float *raw = smem + warp * C::WARP_FLOATS;           // [2][4][6][RS], thread-private entries
+#if !ATON_V4_YSHFL
     float *wyp = raw + 2 * C::RAW_BUF;                   // [4][4][32] plus terms
     float *wym = wyp + C::W_SIGN;                        //            minus terms
-    int *qi = reinterpret_cast<int *>(wym + C::W_SIGN);  // [V4_QCAP] ids of deferred cells + 4 statistics words
-    int qn = 0;                                          // ids queued (warp-uniform)
-    if (lane < 4) qi[V4_QCAP + lane] = 0;
-    __syncwarp();
+#endif
 
     // planes [zb, ze) are advanced: the whole periodic grid (0, nz), or a slab's own planes (1, nz - 1) whose
     // ghost planes 0 and nz - 1 hold the neighbours' boundary planes (no wrap is ever taken then)
@@ -113,7 +118,13 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
     const int rowoff = (y0 + r) * g.nx + x0 + 4 * q;     // own quad inside a plane
     // y halo row of this lane: rows 0 / 3 take the row below / above the tile (others: a harmless re-read)
     const bool hbot = r == 0, htop = r == C::WY - 1;
+#if ATON_V4_YSHFL
+    // roles swapped for the rotation shuffles: the lanes of the TOP row close the row BELOW the tile (its U + F_y goes
+    // to row 0), the lanes of row 0 the row ABOVE (its U - F_y goes to the top row)
+    const int jh = htop ? (y0 == 0 ? g.ny - 1 : y0 - 1) : (hbot ? (y0 + C::WY == g.ny ? 0 : y0 + C::WY) : y0 + r);
+#else
     const int jh = hbot ? (y0 == 0 ? g.ny - 1 : y0 - 1) : (htop ? (y0 + C::WY == g.ny ? 0 : y0 + C::WY) : y0 + r);
+#endif
     const int hoff = jh * g.nx + x0 + 4 * q;
     const int hslot = hbot ? 0 : (htop ? C::WY + 1 : r + 1);
     // x halo cell of this lane: q = 0 the cell left of the tile, q = 7 the cell right of it
@@ -202,6 +213,52 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
             }
         }
         Quad t;
+#if ATON_V4_YSHFL
+        // ---- start plane m from its own state and the +z term carried from plane m-1
+#pragma unroll
+        for (int p = 0; p < 2; p++)
+#pragma unroll
+            for (int v = 0; v < 4; v++) t.v[p][v] = fma2(u.v[p][v], c.keep, zup.v[p][v]);
+        if (INPL) {
+            // ---- y: every lane sends (U + F_y) of its row to the row above and (U - F_y) to the row below by rotation
+            //      shuffles; the top-row lanes send the closed row below the tile instead (it reaches row 0), the row-0
+            //      lanes the closed row above the tile (it reaches the top row)
+            const float4 hn4 = *reinterpret_cast<const float4 *>(buf + myh);
+            const float4 hgx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + myh);
+            const float4 hgy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + myh);
+            const float4 hgz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + myh);
+            const int from_below = (lane + 32 - WXQ) & 31, from_above = (lane + WXQ) & 31;
+            const f2 sg = splat(htop ? 1.0f : -1.0f);
+#pragma unroll
+            for (int p = 0; p < 2; p++) {
+                f2 F[4], e[4] = {ld_pair(hn4, p), ld_pair(hgx4, p), ld_pair(hgy4, p), ld_pair(hgz4, p)}, ea, es, Fh[4];
+                flux_row(1, u.v[p], a[p], s[p], F);
+                closure2(e[0], e[1], e[2], e[3], ea, es);
+                flux_row(1, e, ea, es, Fh);
+#pragma unroll
+                for (int v = 0; v < 4; v++) {
+                    const f2 w = fma2(Fh[v], sg, e[v]);
+                    const f2 P = u.v[p][v] + F[v], M = u.v[p][v] - F[v];
+                    const float sp0 = htop ? lo(w) : lo(P), sp1 = htop ? hi(w) : hi(P);
+                    const float sm0 = hbot ? lo(w) : lo(M), sm1 = hbot ? hi(w) : hi(M);
+                    const f2 yp = pk(__shfl_sync(0xffffffffu, sp0, from_below), __shfl_sync(0xffffffffu, sp1, from_below));
+                    const f2 ym = pk(__shfl_sync(0xffffffffu, sm0, from_above), __shfl_sync(0xffffffffu, sm1, from_above));
+                    t.v[p][v] = fma2(yp + ym, c.h, t.v[p][v]);
+                }
+            }
+        }
+        // ---- z: complete plane m-1, seed plane m+1
+#pragma unroll
+        for (int p = 0; p < 2; p++) {
+            f2 F[4];
+            flux_row(2, u.v[p], a[p], s[p], F);
+#pragma unroll
+            for (int v = 0; v < 4; v++) {
+                pend.v[p][v] = fma2(u.v[p][v] - F[v], c.h, pend.v[p][v]);
+                zup.v[p][v] = (u.v[p][v] + F[v]) * c.h;
+            }
+        }
+#else
         if (INPL) {
             __syncwarp();                                // every lane has consumed the previous plane's y terms
             // ---- y: publish (U + F_y) for the row above, (U - F_y) for the row below
@@ -271,6 +328,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
                 zup.v[p][v] = (u.v[p][v] + F[v]) * c.h;
             }
         }
+#endif
         // ---- x: (U + F_x) of the cell to the left, (U - F_x) of the cell to the right
         if (INPL) {
             f2 Wp[2][4], Wm[2][4];
@@ -332,16 +390,11 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
             ATON_ST4(f.x, xs[0], xs[1]);
             ATON_ST4(f.T, Ts[0], Ts[1]);
 #undef ATON_ST4
-            if (__any_sync(0xffffffffu, nib != 0u)) {     // rare: queue the ids of the deferred cells
-#pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    const bool d = (nib >> j) & 1u;
-                    const unsigned bal = __ballot_sync(0xffffffffu, d);
-                    if (d) qi[qn + __popc(bal & ((1u << lane) - 1u))] = oprev + j;
-                    qn += __popc(bal);
-                }
-            }
+            if (nib) atomicOr(f.defer_mask + ((unsigned)oprev >> 5), nib << (oprev & 31));
         }
+#if ATON_V4_YSHFL
+        pend = t;
+#else
         // ---- y terms of plane m, written straight into the carried registers
         if (INPL) {
             const int rp = r * C::WX + 4 * q;
@@ -356,10 +409,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
         } else {
             pend = t;
         }
-        if (FIN && qn >= 32) {                           // redo 32 deferred cells at a time (warp-uniform branch)
-            __syncwarp();                                // the stores of this and earlier planes are ordered before the redo
-            qn = v4_fix_drain<FLAGS>(fa, qi, qn, 32);
-        }
+#endif
         oprev = ocur;
         kcur = kcur + 1 == g.nz ? 0 : kcur + 1;
         ocur = kcur * plane + rowoff;
@@ -373,19 +423,6 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, const FixArgs *fa, int lz, int z
     iter(yes, no, true, true);                 // m = 1: first own plane, nothing to finish yet
     while (m <= lzn) iter(yes, yes, true, true);   // steady state (the last one stages the z halo plane above)
     iter(no, yes, false, false);               // m = lzn + 1: z halo plane above, finishes plane lzn
-    if (qn > 0) {
-        __syncwarp();
-        v4_fix_drain<FLAGS>(fa, qi, qn, 1);
-    }
-    if (lane == 0) {
-        const int *wst = qi + V4_QCAP;
-        if (wst[2] > 0) {
-            atomicAdd(f.stats, (unsigned long long)wst[0]);
-            atomicMax(f.stats + 1, (unsigned long long)wst[1]);
-            atomicAdd(f.stats + 2, (unsigned long long)wst[2]);
-            if (wst[3] > 0) atomicAdd(f.stats + 3, (unsigned long long)wst[3]);
-        }
-    }
 }
 
 // tile shapes: 32 x 4 (nx % 32 == 0, ny % 4 == 0; the default: 13.8 ms per 1024^3 step) or 64 x 2 (nx % 64 == 0,
@@ -412,24 +449,24 @@ inline int v4_default_lz(const Grid &g, int tile_z, int nzr) {
 }
 
 template <int FLAGS, int WXQ>
-cudaError_t launch_step_v4_wxq(const FieldsIO &f, const Grid &g, const StepConst &c, const FixArgs *fa, int tile_z,
-                               cudaStream_t stream, int zb, int ze) {
+cudaError_t launch_step_v4_wxq(const FieldsIO &f, const Grid &g, const StepConst &c, int tile_z, cudaStream_t stream,
+                               int zb, int ze) {
     using C = V4Cfg<WXQ>;
     // the attribute is per device, not per process: set it at every launch (a cheap driver call)
     cudaError_t e = cudaFuncSetAttribute(step_v4_kernel<FLAGS, WXQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     const int lz = v4_default_lz<WXQ>(g, tile_z, ze - zb);
     const dim3 grid((g.nx / C::WX + C::WARPS - 1) / C::WARPS, g.ny / C::WY, (ze - zb + lz - 1) / lz);
-    step_v4_kernel<FLAGS, WXQ><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, fa, lz, zb, ze);
+    step_v4_kernel<FLAGS, WXQ><<<grid, C::THREADS, C::SMEM, stream>>>(f, g, c, lz, zb, ze);
     return cudaGetLastError();
 }
 
 // wxq must come from v4_pick_wxq (non-zero); planes [zb, ze) are advanced
 template <int FLAGS>
-cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, const FixArgs *fa, int wxq, int tile_z,
-                           cudaStream_t stream, int zb, int ze) {
-    if (wxq == 8) return launch_step_v4_wxq<FLAGS, 8>(f, g, c, fa, tile_z, stream, zb, ze);
-    return launch_step_v4_wxq<FLAGS, 16>(f, g, c, fa, tile_z, stream, zb, ze);
+cudaError_t launch_step_v4(const FieldsIO &f, const Grid &g, const StepConst &c, int wxq, int tile_z, cudaStream_t stream,
+                           int zb, int ze) {
+    if (wxq == 8) return launch_step_v4_wxq<FLAGS, 8>(f, g, c, tile_z, stream, zb, ze);
+    return launch_step_v4_wxq<FLAGS, 16>(f, g, c, tile_z, stream, zb, ze);
 }
 
 }  // namespace aton

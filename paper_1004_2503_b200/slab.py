@@ -6,8 +6,9 @@ into z slabs -- a halo is then one contiguous nx*ny plane per field -- and the p
 `aton_halo_pack` gathers a slab's first / last plane of N, Gx, Gy, Gz into two buffers, `exchange_halos` moves
 them to the neighbours (NCCL send/recv over NVLink; a copy when a rank is its own neighbour), and
 `aton_halo_unpack` writes the received planes into the ghost planes the step kernel reads.  Chemistry is local;
-the diagnostics need one all-reduce of 14 doubles.  Everything numerical runs in libaton.so: this module only
-decides who sends which buffer to whom.
+the diagnostics need one all-reduce of 15 doubles.  Everything numerical runs in libaton.so (also the global mean
+density and the means of the diagnostics: aton_set_mean_from_sums, aton_diag_from_sums): this module only decides who
+sends which buffer to whom and which entries add, max or min.
 """
 from __future__ import annotations
 
@@ -56,23 +57,19 @@ def exchange_halos(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.
         r.wait()
 
 
-def combine_sums(local: List[float], group=None, world: int = 1) -> Dict[str, float]:
-    """All-reduce aton_reduce_sums across the slabs (entries 0-10 sum, 11-12 max, 13 min) -> global diagnostics
-    with the keys of aton_diag_t that can be formed from them (the rates need c*sigma_n: see SlabAton.reduce)."""
+def combine_sums(local: List[float], group=None, world: int = 1) -> List[float]:
+    """All-reduce aton_reduce_sums across the slabs: entries 0-10 and 14 add, 11-12 take the max, 13 the min.  Returns the
+    combined raw sums; the library forms the diagnostics from them (aton_diag_from_sums)."""
     t = torch.tensor(local, dtype=torch.float64)
     if world > 1:
         dev = "cuda" if dist.get_backend(group) == "nccl" else "cpu"
-        s, mx, mn = t[:11].to(dev), t[11:13].to(dev), t[13:].to(dev)
+        s, mx, mn = torch.cat([t[:11], t[14:15]]).to(dev), t[11:13].to(dev), t[13:14].to(dev)
         dist.all_reduce(s, op=dist.ReduceOp.SUM, group=group)
         dist.all_reduce(mx, op=dist.ReduceOp.MAX, group=group)
         dist.all_reduce(mn, op=dist.ReduceOp.MIN, group=group)
-        t = torch.cat([s.cpu(), mx.cpu(), mn.cpu()])
-    v = t.tolist()
-    n = v[0]
-    return {"cells": n, "x_vol": v[1] / n, "x_mass": v[2] / v[3], "nH_mean": v[3] / n, "N_vol": v[4] / n,
-            "N_mass": v[5] / v[3], "T_vol": v[6] / n, "frac_x_half": v[7] / n, "n_nonfinite": int(v[8]),
-            "subcycles_total": int(v[9]), "cells_subcycled": int(v[10]), "f_max": v[11], "subcycles_max": int(v[12]),
-            "N_min": v[13]}
+        s = s.cpu()
+        t = torch.cat([s[:11], mx.cpu(), mn.cpu(), s[11:12]])
+    return t.tolist()
 
 
 class SlabAton:
@@ -88,12 +85,9 @@ class SlabAton:
                     for k in ("send_lo", "send_hi", "recv_lo", "recv_hi")}
 
     def set_fields(self, nH, x, T, N=None, Fx=None, Fy=None, Fz=None):
-        # <n_H> of the linear clumping law is a global mean
-        s = torch.stack([nH.double().sum(), torch.tensor(float(nH.numel()), dtype=torch.float64, device=nH.device)])
-        if self.world > 1:
-            dist.all_reduce(s, group=self.group)
-        self.ctx.set_mean_density(float(s[0] / s[1]))
         self.ctx.set_fields(nH, x, T, N, Fx, Fy, Fz)
+        # <n_H> of the linear clumping law is a GLOBAL mean: all-reduce the library's own sums, hand them back
+        self.ctx.set_mean_from_sums(combine_sums(self.ctx.reduce_sums(), self.group, self.world))
 
     def set_sources(self, pos, rate):
         self.ctx.set_sources(pos, rate)          # global positions; the library keeps this slab's sources
@@ -110,10 +104,8 @@ class SlabAton:
         return self.ctx.get_fields(**kw)
 
     def reduce(self) -> Dict[str, float]:
-        d = combine_sums(self.ctx.reduce_sums(), self.group, self.world)
-        cs = (self.params.get("c_cm_s", 0.0) or 2.99792458e10) * self.params["sigma_n"]
-        d["gamma_vol"], d["gamma_mass"] = cs * d["N_vol"], cs * d["N_mass"]
-        return d
+        """Global diagnostics: the slabs' raw sums all-reduced, the means formed by the library."""
+        return self.ctx.diag_from_sums(combine_sums(self.ctx.reduce_sums(), self.group, self.world))
 
     def close(self):
         self.ctx.close()

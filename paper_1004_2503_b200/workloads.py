@@ -62,7 +62,7 @@ def default_params() -> Dict[str, float]:
     """PAPER.md:L89 single-group constants; every switch off except case-B recombination."""
     return dict(c_cm_s=C_CM_S, sigma_n=2.93e-18, sigma_e=2.49e-18, e_photon_eV=20.27,
                 recomb_case=1, cooling=1, coll_ion=1, clump_model=0, clump_a=1.0, clump_b=2.0,
-                redshift=-1.0, eps_sub=0.1, max_sub=1 << 14, clump_i_a=0.0, clump_i_b=0.0)
+                redshift=-1.0, eps_sub=0.1, max_sub=1 << 14, clump_i_a=0.0, clump_i_b=0.0, flux=0)
 
 
 # ----------------------------------------------------------------------------------------------

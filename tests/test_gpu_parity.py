@@ -493,7 +493,10 @@ def _onestep_check(orc, w, origins, size, k_warm, nH_mean):
                         bad.append((org, nsrc, k, float(e[kk, jj, ii]), c0,
                                     {f: (float(g[f][kk, jj, ii]), float(getattr(ref, f)[kk, jj, ii])) for f in ("x", "T", "N")}))
             bad.append((org, nsrc, "max-rel", err, int(st.sub_max)))
-    assert not bad, bad
+    for b in bad:
+        print("1-step bar violated:", b)
+    print("1-step check:", {k: diag[k] for k in ("cells_subcycled", "cells_fp64", "subcycles_max")}, "worst", worst)
+    assert not bad, bad[-1]
     return worst, diag
 
 

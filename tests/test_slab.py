@@ -42,12 +42,12 @@ for _ in range(3):                                                 # repeated ex
     below, above = slab.neighbours(world, rank)
     assert bool((recv_lo == 10 * below + 2).all()), (rank, recv_lo[0, 0, 0])      # last plane of the slab below
     assert bool((recv_hi == 10 * above + 1).all()), (rank, recv_hi[0, 0, 0])      # first plane of the slab above
-sums = [10.0 + rank, 1.0 * rank, 2.0, 4.0, 0, 0, 0, 0, 0, 5, 1, 0.1 * (rank + 1), 3 + rank, -float(rank)]
+sums = [10.0 + rank, 1.0 * rank, 2.0, 4.0, 0, 0, 0, 0, 0, 5, 1, 0.1 * (rank + 1), 3 + rank, -float(rank), 7.0]
 d = slab.combine_sums(sums, None, world)
 tot = sum(10.0 + r for r in range(world))
-assert abs(d["cells"] - tot) < 1e-12 and abs(d["x_vol"] - sum(range(world)) / tot) < 1e-12
-assert abs(d["x_mass"] - 2.0 * world / (4.0 * world)) < 1e-12 and d["subcycles_total"] == 5 * world
-assert abs(d["f_max"] - 0.1 * world) < 1e-12 and d["subcycles_max"] == 2 + world and d["N_min"] == -(world - 1)
+assert len(d) == 15 and abs(d[0] - tot) < 1e-12 and abs(d[1] - sum(range(world))) < 1e-12        # entries 0-10, 14 add
+assert d[2] == 2.0 * world and d[3] == 4.0 * world and d[9] == 5 * world and d[10] == world and d[14] == 7.0 * world
+assert abs(d[11] - 0.1 * world) < 1e-12 and d[12] == 2 + world and d[13] == -(world - 1)      # 11-12 max, 13 min
 dist.destroy_process_group()
 print("ok", rank)
 """
@@ -123,11 +123,13 @@ def test_slabs_on_one_gpu_equal_the_undivided_run(shape, world):
         sums[:11] += v[:11]
         sums[11:13] = np.maximum(sums[11:13], v[11:13])
         sums[13] = v[13] if s.rank == 0 else min(sums[13], v[13])
-        if world == 1:                                    # the class's own step / reduce path (self-exchange)
-            pass
-        s.close()
-    d = slab.combine_sums(list(sums))
-    assert d["cells"] == nx * ny * nz and d["n_nonfinite"] == 0
+        sums[14] += v[14]
+        if s.rank > 0:
+            s.close()
+    d = ranks[0].ctx.diag_from_sums(list(sums))           # the library forms the means from the combined sums
+    ranks[0].close()
+    assert sums[0] == nx * ny * nz and d["n_nonfinite"] == 0
+    assert d["gamma_vol"] == pytest.approx(dref["gamma_vol"], rel=1e-12) and d["photons_total"] == pytest.approx(dref["photons_total"], rel=1e-12)
     assert d["x_vol"] == pytest.approx(dref["x_vol"], rel=1e-12) and d["x_mass"] == pytest.approx(dref["x_mass"], rel=1e-12)
     assert d["T_vol"] == pytest.approx(dref["T_vol"], rel=1e-12) and d["f_max"] == pytest.approx(dref["f_max"], rel=1e-12)
     assert d["subcycles_total"] == dref["subcycles_total"] and d["cells_subcycled"] == dref["cells_subcycled"]
