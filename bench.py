@@ -39,13 +39,14 @@ def measured_hbm_peak():
         return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
-def recorded_traffic(n):
-    """dram bytes per launch of the step kernel from the committed ncu --set full capture, if any."""
+def recorded_traffic(n, state):
+    """dram bytes per launch of the step kernel from the committed ncu --set full capture of the shipped kernel
+    (profiles/traffic.txt, written from profiles/r02_*), if there is one for this grid and state."""
     p = os.path.join(ROOT, "profiles", "traffic.txt")
     try:
         for line in open(p):
             k, _, v = line.partition(":")
-            if k.strip() == f"dram_bytes_per_launch_n{n}":
+            if k.strip() == f"dram_bytes_per_launch_n{n}_{state}":
                 return float(v.split()[0])
     except Exception:
         pass
@@ -128,12 +129,15 @@ def aggregate(local_ms_total: float, local_units: float, steps: int, world: int)
 
 
 # ------------------------------------------------------------------------------------------ oracle
-def oracle_sample(cfg, n_sample, steps, warm):
+def oracle_sample(cfg, n_sample, steps, warm, threads=0):
     """Time the fp64 oracle, as it stands, on a down-sized twin of the workload (same dx, density
-    statistics and source density): `warm` untimed + `steps` timed steps.  Returns cell-updates/s."""
+    statistics and source density): `warm` untimed + `steps` timed steps on `threads` host threads (0 = all).
+    Returns cell-updates/s."""
     from oracle import aton_oracle as orc
     from paper_1004_2503_b200 import workloads as wl
     orc.build()
+    all_threads = orc.get_threads()
+    orc.set_threads(threads if threads > 0 else all_threads)
     w = wl.make_config(cfg, n=n_sample)
     st, p = orc.from_workload(w)
     pos, rate = w.src_pos.numpy(), w.src_rate.numpy()
@@ -142,7 +146,9 @@ def oracle_sample(cfg, n_sample, steps, warm):
     t0 = time.perf_counter()
     orc.step(st, p, w.dt, steps, pos, rate)
     dt = time.perf_counter() - t0
-    return n_sample ** 3 * steps / dt, dt, orc.get_threads()
+    used = orc.get_threads()
+    orc.set_threads(all_threads)
+    return n_sample ** 3 * steps / dt, dt, used
 
 
 def run_reference(args, rank, world):
@@ -168,6 +174,58 @@ def run_reference(args, rank, world):
 
 
 # ------------------------------------------------------------------------------------------ ours
+def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0):
+    """W untimed + K timed steps (device time, barrier + synchronize on both sides), then the same K steps again with
+    the library's own events around each kernel.  Returns a dict of this rank's numbers."""
+    import torch
+    do_step(dt, warmup)
+    torch.cuda.synchronize()
+    if world > 1:
+        torch.distributed.barrier()
+    sampler = ClockSampler(sampler_rank0) if sampler_rank0 is not None else None
+    l0 = a.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    do_step(dt, steps)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        torch.distributed.barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = a.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    d0 = a.reduce()
+    # the kernels alone: CUDA events on the library's stream around each launch (aton_set_timing), in a second pass
+    # of the same K steps so the events stay out of `value`
+    a.set_timing(True)
+    do_step(dt, steps)
+    k_ms, k_n = a.kernel_time()
+    f_ms, s_ms, f_n = a.fixup_time()
+    a.set_timing(False)
+    d1 = a.reduce()
+    per = lambda k: (d1[k] - d0[k]) / max(steps, 1)
+    return {"ms_total": ms_total, "launches": launches, "clocks": clocks, "diag": d0,
+            "kernel_ms": k_ms / max(k_n, 1), "kernel_launches": k_n,
+            "fixup_ms": f_ms / max(f_n, 1), "stiff_ms": s_ms / max(f_n, 1),
+            "cells_redone_per_step": per("cells_subcycled"), "cells_fp64_per_step": per("cells_fp64"),
+            "x_vol_end": d1["x_vol"]}
+
+
+def roofline_of(leg, cells, steps, peak, peak_src, traffic, kernel_name):
+    achieved = BYTES_PER_CELL_UPDATE * cells / (leg["kernel_ms"] * 1e-3) / 1e9
+    step_ms = leg["ms_total"] / steps
+    achieved_step = BYTES_PER_CELL_UPDATE * cells / (step_ms * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": traffic, "kernel": kernel_name, "kernel_ms": leg["kernel_ms"],
+            "kernel_launches_timed": leg["kernel_launches"], "kernel_share_of_step": leg["kernel_ms"] / step_ms,
+            "fixup_ms": leg["fixup_ms"], "stiff_ms": leg["stiff_ms"],
+            "frac_step": achieved_step / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
+            "frac_step_of_nominal_8TBs": achieved_step / 8000.0,
+            "target_60pct_of_8TBs_met": bool(achieved_step / 8000.0 >= 0.6),
+            "algorithmic_bytes_per_launch": BYTES_PER_CELL_UPDATE * cells, "peak_source": peak_src}
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
@@ -177,64 +235,53 @@ def run_ours(args, rank, world, local_rank):
     build.build()
     cfg = args.config
     n = args.n or {1: 32, 2: 128, 3: 256, 4: 512, 5: 1024}[cfg]
-    w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
-    if args.state == "warm":
-        w = wl.synthetic_warm_state(w)
     variant = 4 if args.variant is None else args.variant
-    if args.decomp == "slab":
-        # ONE box of n x n x (n * world) cells cut into z slabs, one per rank, halo planes exchanged every step
-        # (NEXT-1); each rank generates its own n^3 part of the density and its sources
+    slab_mode = args.decomp == "slab"
+    if slab_mode:
+        # ONE box cut into z slabs, one per rank, halo planes exchanged every step inside the library (aton_step_slab:
+        # NCCL send/recv beside the interior planes, NEXT-1).
+        #   --strong: THE config's box (n^3, e.g. the 1024^3 of config 5) cut N ways -> strong scaling;
+        #   default:  an n x n x (n N) box, every rank generating its own n^3 part -> weak scaling.
         from paper_1004_2503_b200 import slab
-        sl = slab.SlabAton(n, n, n * world, w.box_cm, w.params, rank, world)
-        sl.set_fields(w.nH, w.x, w.T, w.N, w.Fx, w.Fy, w.Fz)
-        pos = w.src_pos.clone()
-        pos[:, 2] = (pos[:, 2] + rank) / world
-        sl.set_sources(pos.contiguous(), w.src_rate.contiguous())
+        if args.strong:
+            w = wl.make_config(cfg, n=n, device="cuda")               # every rank builds the same seeded box ...
+            zb, nzl = slab.slab_range(n, world, rank)                  # ... and keeps its planes
+            sl = slab.SlabAton(n, n, n, w.box_cm, w.params, rank, world, native=True)
+            part = [t[zb:zb + nzl].contiguous() for t in w.fields()]
+            sl.set_fields(*part)
+            sl.set_sources(w.src_pos.contiguous(), w.src_rate.contiguous())
+            del part
+            cells = float(n) * n * nzl
+        else:
+            w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
+            sl = slab.SlabAton(n, n, n * world, w.box_cm, w.params, rank, world, native=True)
+            sl.set_fields(w.nH, w.x, w.T, w.N, w.Fx, w.Fy, w.Fz)
+            pos = w.src_pos.clone()
+            pos[:, 2] = (pos[:, 2] + rank) / world
+            sl.set_sources(pos.contiguous(), w.src_rate.contiguous())
+            cells = float(n) ** 3
         a, do_step = sl.ctx, sl.step
     else:
+        w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
+        if args.state == "warm":
+            w = wl.synthetic_warm_state(w)
         a = aton.from_workload(w)
         a.set_kernel(variant, args.tile_y, args.tile_z)
         do_step = a.step
-    cells = float(n) ** 3
+        cells = float(n) ** 3
     stream = torch.cuda.current_stream()
 
-    # ---- device-resident timing: inputs already in HBM, aton_step only
-    do_step(w.dt, args.warmup)
-    torch.cuda.synchronize()
-    if world > 1:
-        torch.distributed.barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    l0 = a.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record(stream)
-    do_step(w.dt, args.steps)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    if world > 1:
-        torch.distributed.barrier()
-    ms_total = e0.elapsed_time(e1)
-    launches = a.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
-    diag = a.reduce()
-    value, ms_per_step = aggregate(ms_total, cells * args.steps, args.steps, world)
-
-    # ---- the dominant kernel alone: CUDA events on the library's stream around each of its launches
-    #      (aton_set_timing), in a second pass of the same K steps so the events stay out of `value`
-    a.set_timing(True)
-    do_step(w.dt, args.steps)
-    k_ms_total, k_n = a.kernel_time()
-    a.set_timing(False)
-    kernel_ms = k_ms_total / max(k_n, 1)
+    # ---- leg 1 (the headline): device-resident timing, inputs already in HBM, aton_step only
+    leg = timed_leg(a, do_step, w.dt, args.steps, args.warmup, world, stream, local_rank if rank == 0 else None)
+    value, ms_per_step = aggregate(leg["ms_total"], cells * args.steps, args.steps, world)
 
     # ---- end to end through the C ABI with host buffers (upload ICs, K steps, download the state)
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not slab_mode:
         host = {k: torch.empty((n, n, n), dtype=torch.float32, pin_memory=True) for k in ("nH", "x", "T")}
         for k, src in (("nH", w.nH), ("x", w.x), ("T", w.T)):
             host[k].copy_(src)
         out = {k: torch.empty((n, n, n), dtype=torch.float32, pin_memory=True) for k in ("x", "T", "N", "Fx", "Fy", "Fz")}
-        del w.nH, w.x, w.T
         torch.cuda.synchronize()
         if world > 1:
             torch.distributed.barrier()
@@ -249,36 +296,60 @@ def run_ours(args, rank, world, local_rank):
         e2e = {"value": v_e2e, "unit": UNIT, "h2d_bytes_per_step": 3 * 4 * cells / args.steps,
                "d2h_bytes_per_step": 6 * 4 * cells / args.steps, "ms_total": t_e2e,
                "what": "aton_set_fields(host nH,x,T) + aton_step(K) + aton_get_fields(host x,T,N,F), pinned buffers"}
+        del host, out
+
+    # ---- leg 2: the same grid from the synthetic warm state (fronts everywhere, ~10 % of the cells sub-cycle): what a
+    #      front-dominated step costs.  Reported beside the headline, never instead of it.
+    warm = None
+    if not args.no_warm and not slab_mode and args.state == "dark":
+        ww = wl.synthetic_warm_state(w)
+        a.set_fields(*[t.contiguous() for t in ww.fields()])
+        del ww
+        torch.cuda.empty_cache()
+        warm_steps = min(args.steps, args.warm_steps)
+        warm = timed_leg(a, do_step, w.dt, warm_steps, args.warmup, world, stream, None)
+        warm["steps"] = warm_steps
     a.close()
     if rank != 0:
         return
 
     peak, peak_src = measured_hbm_peak()
-    achieved = BYTES_PER_CELL_UPDATE * cells / (kernel_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": recorded_traffic(n),
-                "kernel": {0: "step_ref_kernel", 1: "step_tiled_kernel", 2: "step_fused_kernel", 3: "step_v3_kernel", 4: "step_v4_kernel"}[variant],
-                "kernel_ms": kernel_ms, "kernel_launches_timed": k_n,
-                "kernel_share_of_step": kernel_ms / (ms_total / args.steps), "algorithmic_bytes_per_launch": BYTES_PER_CELL_UPDATE * cells,
-                "peak_source": peak_src}
+    kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel"}[variant]
+    roofline = roofline_of(leg, cells, args.steps, peak, peak_src, recorded_traffic(n, "dark"), kname)
+    extra = {}
+    if warm:
+        extra["ms_per_step_warm"] = warm["ms_total"] / warm["steps"]
+        extra["roofline_warm"] = roofline_of(warm, cells, warm["steps"], peak, peak_src, recorded_traffic(n, "warm"), kname)
+        extra["state_warm"] = {"state": f"workloads.synthetic_warm_state + {args.warmup} warm-up steps, {warm['steps']} timed",
+                               "x_vol_end": warm["x_vol_end"], "cells_redone_per_step": warm["cells_redone_per_step"],
+                               "cells_fp64_per_step": warm["cells_fp64_per_step"], "subcycles_max": warm["diag"]["subcycles_max"]}
     cpu = None
     if not args.no_cpu:
         v, secs, cores = oracle_sample(cfg, args.cpu_sample_n, args.cpu_sample_steps, 3)
+        n1 = max(32, args.cpu_sample_n // 2)
+        v1, secs1, _ = oracle_sample(cfg, n1, max(4, args.cpu_sample_steps // 4), 2, threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                "sample": f"config {cfg} twin at {args.cpu_sample_n}^3 (same dx, density statistics, source density), "
-                         f"{args.cpu_sample_steps} steps after 3 warm-up, fp64, gcc -O2 + OpenMP"}
+                         f"{args.cpu_sample_steps} steps after 3 warm-up, fp64, gcc -O2 + OpenMP",
+               "value_1thread": v1, "seconds_1thread": secs1,
+               "sample_1thread": f"the same twin at {n1}^3, {max(4, args.cpu_sample_steps // 4)} steps after 2 warm-up, one thread"}
+    diag = leg["diag"]
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "strong" if (slab_mode and args.strong) else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config {cfg}: {n}^3 periodic box, lognormal density, {int(w.src_rate.numel())} sources, "
                                    f"physics flags {dict((k, w.params[k]) for k in ('recomb_case', 'cooling', 'coll_ion', 'clump_model'))}",
                        "state": args.state + f" start + {args.warmup} warm-up steps",
                        "l2": "working set per step (52 B/cell) exceeds the 126 MB L2" if 52 * cells > 4 * 126e6 else "fits in L2 (latency bound; not an HBM figure)",
-                       "parallelism": ("z slabs of one box, halo planes exchanged every step" if args.decomp == "slab"
+                       "parallelism": (("z slabs of the one box (strong scaling)" if args.strong else "z slabs of one n x n x (n N) box")
+                                       + ", halo planes exchanged every step inside the library, overlapped" if slab_mode
                                        else "replicas" if world > 1 else "single GPU"),
                        "x_vol_end": diag["x_vol"], "subcycles_per_cell_step": diag["subcycles_total"] / cells / max(diag["steps_done"], 1),
-                       "subcycles_max": diag["subcycles_max"], "n_nonfinite": diag["n_nonfinite"]},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks}
+                       "subcycles_max": diag["subcycles_max"], "n_nonfinite": diag["n_nonfinite"],
+                       "cells_redone_per_step": leg["cells_redone_per_step"], "cells_fp64_per_step": leg["cells_fp64_per_step"]},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": leg["launches"], "clocks": leg["clocks"]}
+    line.update(extra)
     print(json.dumps(line), flush=True)
 
 
@@ -296,6 +367,9 @@ def main():
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--tile-y", type=int, default=0)
     ap.add_argument("--tile-z", type=int, default=0)
+    ap.add_argument("--strong", action="store_true", help="--decomp slab: cut the config's own box N ways (strong scaling)")
+    ap.add_argument("--no-warm", action="store_true", help="skip the second (synthetic warm state) leg")
+    ap.add_argument("--warm-steps", type=int, default=50, help="timed steps of the warm leg (at most --steps)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-sample-n", type=int, default=128)

@@ -143,9 +143,9 @@ int aton_set_timing(aton_t *ctx, int on);
 /* Sum [ms] and number of the bracketed launches since aton_set_timing(ctx, 1).  Synchronises. */
 int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches);
 
-/* The same for the second kernel of a step (variant 4: the fp64 redo of stiff cells; variant 2: the fix-up kernel).
- * Variant 4 redoes its sub-cycling cells inside the step kernel, so their cost is part of aton_kernel_time. */
-int aton_fixup_time(aton_t *ctx, double *ms_total, long long *n_launches);
+/* The same for the other two kernels of a step: step_fixup_kernel (the sub-cycling cells and, for variant 4, the source
+ * cells) and step_stiff_kernel (the fp64 redo of the cells whose fp32 sub-cycling is not accurate enough). */
+int aton_fixup_time(aton_t *ctx, double *ms_fixup, double *ms_stiff, long long *n_launches);
 
 /* ---- slab decomposition along z (the paper's multi-GPU mode, PAPER.md:L471-484,
  * re-cut as z slabs whose one-plane halo of (N, F) is one contiguous block per field) ----

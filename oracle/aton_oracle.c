@@ -494,3 +494,111 @@ void orc_reduce(long ncell, const double *N, const double *Fx, const double *Fy,
     out[4] = sN * p->dx * p->dx * p->dx; out[5] = sT / ncell; out[6] = fmax; out[7] = nmin;
     out[8] = nbad; out[9] = nhalf / ncell;
 }
+
+/* =============================================================================================
+ * Analysis and source front end around the step.  Not per step.
+ * ============================================================================================= */
+
+/* ---------------------------------------------------------------------------------------------
+ * Clumping-factor measurement (section 3.2.1): "Clumping factors are computed by averaging the
+ * relevant quantities on these 512 cells" of every b x b x b block (b = 8 in the paper: one cell of the coarse run),
+ *     C_R = <n_H^2 x^2> / <n_H x>^2,          C_I = <n_gamma (1-x) n_H> / ( <n_gamma> <(1-x) n_H> )      (L247),
+ * together with the block's mean density <n_H> and its ionised fraction <n_H x>/<n_H> (what the coarse cell holds;
+ * the paper bins C_R, C_I against these two, Fig.12-13).  Where a denominator vanishes (no ionised gas / no photons /
+ * no neutral gas) the factor is 1 (reading S21: a homogeneous block).  Outputs: [nz/b][ny/b][nx/b].
+ * ------------------------------------------------------------------------------------------- */
+void orc_clumping_blocks(int nx, int ny, int nz, int b, const double *nH, const double *x, const double *N,
+                         double *out_nH, double *out_x, double *out_CR, double *out_CI) {
+    int bx = nx / b, by = ny / b, bz = nz / b;
+    double inv = 1.0 / ((double)b * b * b);
+    for (int K = 0; K < bz; K++)
+        for (int J = 0; J < by; J++)
+            for (int I = 0; I < bx; I++) {
+                double s_n = 0, s_nx = 0, s_n2x2 = 0, s_g = 0, s_yn = 0, s_gyn = 0;
+                for (int k = K * b; k < (K + 1) * b; k++)
+                    for (int j = J * b; j < (J + 1) * b; j++)
+                        for (int i = I * b; i < (I + 1) * b; i++) {
+                            long id = i + (long)nx * (j + (long)ny * k);
+                            double n = nH[id], xx = x[id], g = N[id], yn = (1.0 - xx) * n;
+                            s_n += n; s_nx += n * xx; s_n2x2 += n * n * xx * xx;
+                            s_g += g; s_yn += yn; s_gyn += g * yn;
+                        }
+                long o = I + (long)bx * (J + (long)by * K);
+                double m_n = s_n * inv, m_nx = s_nx * inv, m_g = s_g * inv, m_yn = s_yn * inv;
+                out_nH[o] = m_n;
+                out_x[o] = m_n > 0.0 ? m_nx / m_n : 0.0;
+                out_CR[o] = m_nx > 0.0 ? (s_n2x2 * inv) / (m_nx * m_nx) : 1.0;
+                out_CI[o] = (m_g > 0.0 && m_yn > 0.0) ? (s_gyn * inv) / (m_g * m_yn) : 1.0;
+            }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * 2-D distribution of two per-cell quantities (the J21(n_H), x(n_H), (1-x)(n_H) planes of PAPER.md Fig.5-19; L417
+ * names histogramming as a GPU pattern).  Bin of a value v on an axis: floor((f(v) - lo)/(hi - lo) * nbins) with
+ * f = log10 when `logscale`, v otherwise; values outside [lo, hi) (or <= 0 on a log axis) are not counted but
+ * tallied in *outside.  counts[ib * na + ia].
+ * ------------------------------------------------------------------------------------------- */
+void orc_hist2d(long n, const double *a, const double *b, int log_a, int log_b, double a_lo, double a_hi,
+                double b_lo, double b_hi, int na, int nb, long long *counts, long long *outside) {
+    for (long k = 0; k < (long)na * nb; k++) counts[k] = 0;
+    long long out = 0;
+    for (long i = 0; i < n; i++) {
+        double va = a[i], vb = b[i];
+        if ((log_a && !(va > 0.0)) || (log_b && !(vb > 0.0))) { out++; continue; }
+        double fa = log_a ? log10(va) : va, fb = log_b ? log10(vb) : vb;
+        double ua = (fa - a_lo) / (a_hi - a_lo) * na, ub = (fb - b_lo) / (b_hi - b_lo) * nb;
+        if (!(ua >= 0.0 && ua < (double)na && ub >= 0.0 && ub < (double)nb)) { out++; continue; }
+        counts[(long)floor(ub) * na + (long)floor(ua)]++;
+    }
+    *outside = out;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Source front end (section 2.3, Eq.8-9).  For the transfer from t_p to t_{p+1} only the star
+ * particles of snapshot p+1 are used.  With a_{p+1} the particle's age at t_{p+1}, a_p = a_{p+1} - (t_{p+1} - t_p),
+ * L its lifetime as an ionising source and Ndot its intrinsic rate (photons_per_baryon * n_baryons / L):
+ *   a_p > L                discarded;
+ *   a_p < 0                born in the interval: "diluted" rate  (a_{p+1} / (t_{p+1} - t_p)) Ndot   -- the printed
+ *                          "(a_{p+1} a*)/(t_{p+1} t_p)" lost its minus signs (reading G5): the star shone from its
+ *                          birth a* to t_{p+1}, i.e. for a_{p+1} (at most L), spread over the interval;
+ *   0 <= a_p <= L          min(1, (L - a_p)/(t_{p+1} - t_p)) Ndot  (it may stop shining inside the interval).
+ * Every branch emits, over the interval, exactly the photons the star emits in it.  Then Eq.8: Ndot_eff = Ndot f_esc B
+ * with the boost of Eq.9, read as B = max(1, a_b exp(k_b / t)) (reading G6: it is SFR_converged/SFR_actual >= 1 and
+ * Table 1's a_b, k_b give B ~ 90 at 700 Myr for the 100 Mpc/h box; the printed "min" would switch it off), t = the age of
+ * the Universe at the middle of the interval.
+ * ------------------------------------------------------------------------------------------- */
+double orc_boost(double t, double a_b, double k_b) {
+    double B = a_b * exp(k_b / t);
+    return B > 1.0 ? B : 1.0;
+}
+
+void orc_star_rates(long n, const double *age1, const double *life, const double *nbaryons, double photons_per_baryon,
+                    double t_p, double t_p1, double f_esc, double a_b, double k_b, double *rate) {
+    double dtp = t_p1 - t_p;
+    double B = orc_boost(0.5 * (t_p + t_p1), a_b, k_b);
+    for (long s = 0; s < n; s++) {
+        double L = life[s], ndot = photons_per_baryon * nbaryons[s] / L;
+        double a1 = age1[s], a0 = a1 - dtp, frac;
+        if (a0 > L) frac = 0.0;
+        else if (a0 < 0.0) frac = (a1 < L ? a1 : L) / dtp;
+        else { frac = (L - a0) / dtp; if (frac > 1.0) frac = 1.0; }
+        rate[s] = frac * ndot * f_esc * B;
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Thomson optical depth, Eq.10: tau = c sigma_T int n_e dt with n_e = x n_H, evaluated from a
+ * history (z_i, x_i) of the mass-weighted ionised fraction in a flat LCDM background (the paper's WMAP-5 run, L45):
+ *   n_H(z) = nH0 (1+z)^3,  dt = -dz / ((1+z) H(z)),  H = H0 sqrt(Om (1+z)^3 + 1 - Om)
+ *   tau = c sigma_T nH0 int_0^zmax x(z) (1+z)^2 / H(z) dz   (trapezoid rule over the given points, z ascending).
+ * ------------------------------------------------------------------------------------------- */
+double orc_thomson_tau(long n, const double *z, const double *x, double nH0, double H0, double Om) {
+    const double c = 2.99792458e10, sigma_T = 6.6524587e-25;
+    double tau = 0.0;
+    for (long i = 0; i + 1 < n; i++) {
+        double f0 = x[i] * (1 + z[i]) * (1 + z[i]) / (H0 * sqrt(Om * pow(1 + z[i], 3) + 1.0 - Om));
+        double f1 = x[i + 1] * (1 + z[i + 1]) * (1 + z[i + 1]) / (H0 * sqrt(Om * pow(1 + z[i + 1], 3) + 1.0 - Om));
+        tau += 0.5 * (f0 + f1) * (z[i + 1] - z[i]);
+    }
+    return c * sigma_T * nH0 * tau;
+}

@@ -79,6 +79,14 @@ def lib():
         L.orc_step.argtypes = ([C.c_int] * 3 + [_dp] * 7 + [C.c_long, _dp, _dp, C.c_double, C.c_int,
                                                             C.POINTER(Params), C.POINTER(C.c_longlong)])
         L.orc_reduce.argtypes = [C.c_long] + [_dp] * 7 + [C.POINTER(Params), _dp]
+        L.orc_clumping_blocks.argtypes = [C.c_int] * 4 + [_dp] * 7
+        L.orc_hist2d.argtypes = [C.c_long, _dp, _dp, C.c_int, C.c_int] + [C.c_double] * 4 + [C.c_int, C.c_int,
+                                 C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.orc_boost.restype = C.c_double
+        L.orc_boost.argtypes = [C.c_double] * 3
+        L.orc_star_rates.argtypes = [C.c_long, _dp, _dp, _dp] + [C.c_double] * 6 + [_dp]
+        L.orc_thomson_tau.restype = C.c_double
+        L.orc_thomson_tau.argtypes = [C.c_long, _dp, _dp, C.c_double, C.c_double, C.c_double]
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_threads.restype = C.c_int
         _lib = L
@@ -267,6 +275,46 @@ def reduce(st: State, p: Params) -> Dict[str, float]:
     keys = ("x_vol", "x_mass", "gamma_vol", "gamma_mass", "photons_total", "T_vol", "f_max",
             "N_min", "n_nonfinite", "frac_x_half")
     return dict(zip(keys, out.tolist()))
+
+
+def clumping_blocks(nH, x, N, b: int = 8) -> Dict[str, np.ndarray]:
+    """Clumping-factor measurement over b^3 blocks: dict of [nz/b, ny/b, nx/b] arrays."""
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (nH, x, N)]
+    nz, ny, nx = a[0].shape
+    shape = (nz // b, ny // b, nx // b)
+    out = [np.zeros(shape) for _ in range(4)]
+    lib().orc_clumping_blocks(nx, ny, nz, b, *[_p(v) for v in a], *[_p(v) for v in out])
+    return dict(zip(("nH", "x", "C_R", "C_I"), out))
+
+
+def hist2d(a, b, log_a: bool, log_b: bool, a_range, b_range, na: int, nb: int):
+    """2-D histogram counts[nb, na] and the number of values outside the ranges."""
+    va = np.ascontiguousarray(a, dtype=np.float64).reshape(-1)
+    vb = np.ascontiguousarray(b, dtype=np.float64).reshape(-1)
+    counts = np.zeros((nb, na), dtype=np.int64)
+    outside = C.c_longlong(0)
+    lib().orc_hist2d(va.size, _p(va), _p(vb), int(log_a), int(log_b), float(a_range[0]), float(a_range[1]),
+                     float(b_range[0]), float(b_range[1]), na, nb,
+                     counts.ctypes.data_as(C.POINTER(C.c_longlong)), C.byref(outside))
+    return counts, int(outside.value)
+
+
+def boost(t: float, a_b: float, k_b: float) -> float:
+    return float(lib().orc_boost(float(t), float(a_b), float(k_b)))
+
+
+def star_rates(age1, life, nbaryons, photons_per_baryon, t_p, t_p1, f_esc, a_b, k_b) -> np.ndarray:
+    """Effective emission rates of star particles over [t_p, t_p1] (section 2.3, Eq.8-9)."""
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (age1, life, nbaryons)]
+    out = np.zeros(a[0].size)
+    lib().orc_star_rates(a[0].size, *[_p(v) for v in a], float(photons_per_baryon), float(t_p), float(t_p1),
+                         float(f_esc), float(a_b), float(k_b), _p(out))
+    return out
+
+
+def thomson_tau(z, x, nH0: float, H0: float, Om: float) -> float:
+    zz, xx = [np.ascontiguousarray(v, dtype=np.float64) for v in (z, x)]
+    return float(lib().orc_thomson_tau(zz.size, _p(zz), _p(xx), float(nH0), float(H0), float(Om)))
 
 
 def from_workload(w, nH_mean: Optional[float] = None):

@@ -94,7 +94,7 @@ def load_library(path: Optional[str] = None):
     L.aton_kernel_time.restype = C.c_int
     L.aton_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.aton_fixup_time.restype = C.c_int
-    L.aton_fixup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.aton_fixup_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.aton_init_slab.restype = C.c_int
     L.aton_init_slab.argtypes = [C.POINTER(vp), C.POINTER(Grid), C.POINTER(Box), C.POINTER(Params), vp, C.c_int, C.c_int]
     L.aton_halo_pack.restype = C.c_int
@@ -278,10 +278,10 @@ class Aton:
         return ms.value, n.value
 
     def fixup_time(self):
-        """(sum of ms, launches) of the event-bracketed second kernel of a step since set_timing(True)."""
-        ms, n = C.c_double(), C.c_longlong()
-        self._check(self._L.aton_fixup_time(self._h, C.byref(ms), C.byref(n)))
-        return ms.value, n.value
+        """(ms of step_fixup_kernel, ms of step_stiff_kernel, launches) summed since set_timing(True)."""
+        ms, ms2, n = C.c_double(), C.c_double(), C.c_longlong()
+        self._check(self._L.aton_fixup_time(self._h, C.byref(ms), C.byref(ms2), C.byref(n)))
+        return ms.value, ms2.value, n.value
 
     def launch_count(self) -> int:
         return int(self._L.aton_launch_count(self._h))

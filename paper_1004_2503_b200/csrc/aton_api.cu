@@ -124,6 +124,14 @@ void fix_mark(aton_ctx *ctx) {
     ctx->ev_fix.push_back(e);
 }
 
+void stiff_mark(aton_ctx *ctx) {
+    if (!ctx->timing) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, ctx->stream);
+    ctx->ev_stiff.push_back(e);
+}
+
 template <int FLAGS>
 cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     const StepConst &sc = ctx->sc;
@@ -164,11 +172,13 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     fix_mark(ctx);
     ctx->launches++;
     e = launch_step_fixup<FLAGS>(ctx->fixargs + ctx->cur, (long)ctx->plane * zb, (long)ctx->plane * ze, ctx->stream);
+    fix_mark(ctx);
     if (e == cudaSuccess && (FLAGS & F_COOL)) {       // without cooling nothing sub-cycles: no cell can be stiff
         ctx->launches++;
+        stiff_mark(ctx);
         e = launch_step_stiff<FLAGS>(ctx->fixargs + ctx->cur, ctx->stream);
+        stiff_mark(ctx);
     }
-    fix_mark(ctx);
     return e;
 }
 
@@ -373,6 +383,7 @@ void aton_free(aton_t *ctx) {
     slab_comm_free(ctx);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->ev_stiff) cudaEventDestroy(e);
     for (int b = 0; b < 2; b++)
         for (int v = 0; v < 4; v++) cudaFree(ctx->rad[b][v]);
     cudaFree(ctx->x); cudaFree(ctx->T); cudaFree(ctx->nH);
@@ -401,8 +412,10 @@ int aton_set_timing(aton_t *ctx, int on) {
     if (!ctx) return ATON_EINVAL;
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->ev_stiff) cudaEventDestroy(e);
     ctx->ev.clear();
     ctx->ev_fix.clear();
+    ctx->ev_stiff.clear();
     ctx->timing = on != 0;
     return ATON_OK;
 }
@@ -421,16 +434,19 @@ int aton_kernel_time(aton_t *ctx, double *ms_total, long long *n_launches) {
     return ATON_OK;
 }
 
-int aton_fixup_time(aton_t *ctx, double *ms_total, long long *n_launches) {
-    if (!ctx || !ms_total || !n_launches) return ATON_EINVAL;
+int aton_fixup_time(aton_t *ctx, double *ms_fixup, double *ms_stiff, long long *n_launches) {
+    if (!ctx || !ms_fixup || !ms_stiff || !n_launches) return ATON_EINVAL;
     CU(ctx, cudaStreamSynchronize(ctx->stream));
-    double tot = 0.0;
-    for (size_t i = 0; i + 1 < ctx->ev_fix.size(); i += 2) {
-        float ms = 0.0f;
-        CU(ctx, cudaEventElapsedTime(&ms, ctx->ev_fix[i], ctx->ev_fix[i + 1]));
-        tot += ms;
-    }
-    *ms_total = tot;
+    double tot[2] = {0.0, 0.0};
+    const std::vector<cudaEvent_t> *lists[2] = {&ctx->ev_fix, &ctx->ev_stiff};
+    for (int k = 0; k < 2; k++)
+        for (size_t i = 0; i + 1 < lists[k]->size(); i += 2) {
+            float ms = 0.0f;
+            CU(ctx, cudaEventElapsedTime(&ms, (*lists[k])[i], (*lists[k])[i + 1]));
+            tot[k] += ms;
+        }
+    *ms_fixup = tot[0];
+    *ms_stiff = tot[1];
     *n_launches = (long long)(ctx->ev_fix.size() / 2);
     return ATON_OK;
 }

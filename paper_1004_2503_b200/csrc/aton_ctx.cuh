@@ -58,7 +58,8 @@ struct aton_ctx {
     int variant = 4, tile_y = 0, tile_z = 0;
     bool timing = false;                   // aton_set_timing: CUDA events around the kernels of a step
     std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch of the dominant step kernel
-    std::vector<cudaEvent_t> ev_fix;       // the same for the second kernel of a step (fp64 redo / mask fix-up)
+    std::vector<cudaEvent_t> ev_fix;       // the same for step_fixup_kernel ...
+    std::vector<cudaEvent_t> ev_stiff;     // ... and for step_stiff_kernel
     aton::StepConst sc{};                  // constants of the step size fix_dt (prepare_step)
     aton::StepConstD scd{};
     aton::SlabComm *comm = nullptr;        // aton_comm_init (slab contexts only)

@@ -61,70 +61,87 @@ __global__ void __launch_bounds__(128) step_stiff_kernel(const FixArgs *fa) {
 // shared-memory queue and processed one per thread once the queue holds a few hundred (or the scan ends),
 // so the data-dependent sub-cycle loops run on full warps.  Sources were injected by the step kernel.
 // ---------------------------------------------------------------------------------------------------
-constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS;
+constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS, FIXUP_GROUP = 8;
 
 template <int FLAGS>
 __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
     __shared__ int queue[FIXUP_QCAP];
-    __shared__ int qn;
+    __shared__ int qn, qhead;
     const FieldsIO &f = fa->f;
-    if (threadIdx.x == 0) qn = 0;
+    if (threadIdx.x == 0) { qn = 0; qhead = 0; }
     __syncthreads();
     int nsub_extra = 0, nsub_max = 0, ncell = 0;
-    const int nchunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
-    for (int ch = blockIdx.x; ch < nchunks + (int)gridDim.x; ch += gridDim.x) {
-        const bool scan = ch < nchunks;         // the last trip only drains the queue
-        if (scan) {
-            const int w = word0 + ch * FIXUP_THREADS + threadIdx.x;
-            unsigned bits = w < word0 + nwords ? f.defer_mask[w] : 0u;
-            if (bits) {
+    // redo the queued cells (all threads of the block call this together)
+    auto drain = [&]() {
+        const int n = qn;
+        // self-scheduling: a lane takes the next cell when it is done with its own, so a round lasts as long as its
+        // slowest cell, not as long as the slowest cell of every stride (source cells take tens of sub-cycles)
+        for (int it = atomicAdd(&qhead, 1); it < n; it = atomicAdd(&qhead, 1)) {
+            const int id = queue[it];
+            float N = f.N1[id], gx = f.Gx1[id], gy = f.Gy1[id], gz = f.Gz1[id];
+            float x = f.x[id], T = f.T[id];
+            if (f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) N += source_lookup(f, id, fa->c.dt);
+            const int ns = chemistry<FLAGS, true>(N, gx, gy, gz, x, T, __ldg(f.nH + id), fa->c);
+            if (ns >= 0) {
+                f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
+                f.x[id] = x; f.T[id] = T;
+                nsub_extra += ns - 1;
+                nsub_max = max(nsub_max, ns);
+                ncell++;
+            } else {                        // stiff: the cell keeps its values; step_stiff_kernel redoes it in fp64
+                const unsigned slot = atomicAdd(f.stiff_n, 1u);
+                if (slot < f.stiff_cap) {
+                    f.stiff_q[slot] = id;
+                } else {                    // queue full (the cap is ncell / 16): redo it here
+                    double Nd = (double)f.N1[id] + ((f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) ? source_lookup_d(f, id, fa->cd.dt) : 0.0);
+                    double ax = f.Gx1[id], ay = f.Gy1[id], az = f.Gz1[id], xd = f.x[id], Td = f.T[id];
+                    const int nd = chemistry_f64<FLAGS>(Nd, ax, ay, az, xd, Td, (double)__ldg(f.nH + id), fa->cd);
+                    f.N1[id] = (float)Nd; f.Gx1[id] = (float)ax; f.Gy1[id] = (float)ay; f.Gz1[id] = (float)az;
+                    f.x[id] = (float)xd; f.T[id] = (float)Td;
+                    nsub_extra += nd - 1;
+                    nsub_max = max(nsub_max, nd);
+                    ncell++;
+                    atomicAdd(f.stats + 3, 1ull);
+                }
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) { qn = 0; qhead = 0; }
+        __syncthreads();
+    };
+    // the mask is scanned in groups of FIXUP_GROUP chunks of FIXUP_THREADS words: all the group's words are loaded at
+    // once and an empty group (almost all of them away from fronts and sources) costs one block-wide vote
+    const int end = word0 + nwords;
+    const int ngroups = (nwords + FIXUP_GROUP * FIXUP_THREADS - 1) / (FIXUP_GROUP * FIXUP_THREADS);
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        unsigned bits[FIXUP_GROUP];
+        unsigned any = 0u;
+#pragma unroll
+        for (int k = 0; k < FIXUP_GROUP; k++) {
+            const int w = word0 + (grp * FIXUP_GROUP + k) * FIXUP_THREADS + threadIdx.x;
+            bits[k] = w < end ? f.defer_mask[w] : 0u;
+            any |= bits[k];
+        }
+        if (!__syncthreads_or(any != 0u)) continue;
+#pragma unroll
+        for (int k = 0; k < FIXUP_GROUP; k++) {
+            if (bits[k]) {
+                const int w = word0 + (grp * FIXUP_GROUP + k) * FIXUP_THREADS + threadIdx.x;
                 f.defer_mask[w] = 0u;
-                int pos = atomicAdd(&qn, __popc(bits));
-                while (bits) {
-                    const int b = __ffs(bits) - 1;
-                    bits &= bits - 1;
+                unsigned bb = bits[k];
+                int pos = atomicAdd(&qn, __popc(bb));
+                while (bb) {
+                    const int b = __ffs(bb) - 1;
+                    bb &= bb - 1;
                     queue[pos++] = w * 32 + b;
                 }
             }
-        }
-        __syncthreads();
-        const int n = qn;
-        if (n >= FIXUP_QTHRESH || (!scan && n > 0)) {
-            for (int it = threadIdx.x; it < n; it += FIXUP_THREADS) {
-                const int id = queue[it];
-                float N = f.N1[id], gx = f.Gx1[id], gy = f.Gy1[id], gz = f.Gz1[id];
-                float x = f.x[id], T = f.T[id];
-                if (f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) N += source_lookup(f, id, fa->c.dt);
-                const int ns = chemistry<FLAGS, true>(N, gx, gy, gz, x, T, __ldg(f.nH + id), fa->c);
-                if (ns >= 0) {
-                    f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
-                    f.x[id] = x; f.T[id] = T;
-                    nsub_extra += ns - 1;
-                    nsub_max = max(nsub_max, ns);
-                    ncell++;
-                } else {                        // stiff: the cell keeps its values; step_stiff_kernel redoes it in fp64
-                    const unsigned slot = atomicAdd(f.stiff_n, 1u);
-                    if (slot < f.stiff_cap) {
-                        f.stiff_q[slot] = id;
-                    } else {                    // queue full (the cap is ncell / 16): redo it here
-                        double Nd = (double)f.N1[id] + ((f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) ? source_lookup_d(f, id, fa->cd.dt) : 0.0);
-                        double ax = f.Gx1[id], ay = f.Gy1[id], az = f.Gz1[id], xd = f.x[id], Td = f.T[id];
-                        const int nd = chemistry_f64<FLAGS>(Nd, ax, ay, az, xd, Td, (double)__ldg(f.nH + id), fa->cd);
-                        f.N1[id] = (float)Nd; f.Gx1[id] = (float)ax; f.Gy1[id] = (float)ay; f.Gz1[id] = (float)az;
-                        f.x[id] = (float)xd; f.T[id] = (float)Td;
-                        nsub_extra += nd - 1;
-                        nsub_max = max(nsub_max, nd);
-                        ncell++;
-                        atomicAdd(f.stats + 3, 1ull);
-                    }
-                }
-            }
             __syncthreads();
-            if (threadIdx.x == 0) qn = 0;
+            if (qn >= FIXUP_QTHRESH) drain();         // uniform: every thread reads the same qn after the barrier
         }
-        __syncthreads();
-        if (!scan) break;
     }
+    __syncthreads();
+    if (qn > 0) drain();
     // statistics: warp reduce, one atomic set per warp that saw work
     for (int o = 16; o > 0; o >>= 1) {
         nsub_extra += __shfl_xor_sync(0xffffffffu, nsub_extra, o);
@@ -142,8 +159,8 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
 template <int FLAGS>
 cudaError_t launch_step_fixup(const FixArgs *fa, long cell0, long cell1, cudaStream_t stream) {
     const int word0 = (int)(cell0 / 32), nwords = (int)((cell1 + 31) / 32) - word0;
-    const int nchunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
-    const int blocks = nchunks < 148 * 8 ? nchunks : 148 * 8;
+    const int ngroups = (nwords + FIXUP_GROUP * FIXUP_THREADS - 1) / (FIXUP_GROUP * FIXUP_THREADS);
+    const int blocks = ngroups < 148 * 8 ? (ngroups > 0 ? ngroups : 1) : 148 * 8;
     step_fixup_kernel<FLAGS><<<blocks, FIXUP_THREADS, 0, stream>>>(fa, word0, nwords);
     return cudaGetLastError();
 }

@@ -26,7 +26,8 @@ struct RatesD {
 template <int FLAGS>
 __device__ __noinline__ void rates_f64(double T, const StepConstD &c, RatesD &r) {
     constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL, COLL = FLAGS & F_COLL;
-    const double lam = 315614.0 / T, L = log(lam);                       // lambda = 2 * 157807 K / T
+    const double invT = 1.0 / T, lam = 315614.0 * invT;                  // lambda = 2 * 157807 K / T
+    const double LT = log(T), L = 12.662275226919286 - LT;               // ln lambda = ln 315614 - ln T
     // Hui & Gnedin (1997): alpha = K lam^p / (1 + (lam/l0)^q)^r
     const double uB = exp(0.407 * (L - 1.0079579203999789));                // ln 2.740
     const double aB = 2.753e-14 * exp(1.5 * L - 2.242 * log1p(uB));
@@ -44,30 +45,31 @@ __device__ __noinline__ void rates_f64(double T, const StepConstD &c, RatesD &r)
     double zci = 0.0, zci_t = 0.0;
     if (COLL) {
         const double u = exp(0.874 * (L + 1.0384583658483626));              // -ln 0.354
+        const double l1u = log1p(u);
         // 21.11 T^-1.5 exp(-lam/2) lam^-1.089 / (1+u)^1.101
-        r.beta = 21.11 * exp(-1.5 * log(T) - 0.5 * lam - 1.089 * L - 1.101 * log1p(u));
+        r.beta = 21.11 * exp(-1.5 * LT - 0.5 * lam - 1.089 * L - 1.101 * l1u);
         if (COOL) {
             zci = r.beta * c.zci_over_beta;
-            zci_t = zci * (-1.5 + 0.5 * lam + 1.089 + 1.101 * 0.874 * u / (1.0 + u));
+            zci_t = zci * (-0.411 + 0.5 * lam + 0.962274 * (1.0 - exp(-l1u)));      // u/(1+u) = 1 - 1/(1+u)
         }
     }
     if (COOL) {
         // recombination cooling K T lam^p / (1+u)^r ; d ln/d ln T = 1 - p + r q u/(1+u)
         constexpr double q = CASE_A ? 0.502 : 0.376, ln_l0 = CASE_A ? -0.6143360001356556 : 0.8109302162163288;
         constexpr double p = CASE_A ? 1.965 : 1.970, rr = CASE_A ? 2.697 : 3.720;
-        const double u = exp(q * (L - ln_l0));
-        r.zrec = c.zrec0 * T * exp(p * L - rr * log1p(u));
-        r.zrec_t = r.zrec * (1.0 - p + rr * q * u / (1.0 + u));
+        const double u = exp(q * (L - ln_l0)), iu = 1.0 / (1.0 + u);
+        r.zrec = c.zrec0 * T * exp(p * L + rr * log(iu));
+        r.zrec_t = r.zrec * (1.0 - p + rr * q * u * iu);
         // bremsstrahlung with Gaunt factor 1.1 + 0.34 exp(-(5.5 - log10 T)^2 / 3)
-        const double d = 5.5 - log10(T);
-        const double gau = 0.34 * exp(-d * d / 3.0), gff = 1.1 + gau, sqT = sqrt(T);
+        const double d = 5.5 - LT * 0.4342944819032518;
+        const double gau = 0.34 * exp(d * d * (-1.0 / 3.0)), gff = 1.1 + gau, sqT = sqrt(T);
         r.zff = c.zff0 * gff * sqT;
-        r.zff_t = r.zff * (0.5 + gau * (2.0 * d / 3.0) / 2.302585092994046 / gff);
+        r.zff_t = c.zff0 * sqT * (0.5 * gff + gau * d * 0.2895296546021679);          // (2/3)/ln 10
         // collisional excitation
-        const double pw = sqrt(T * 1.0e-5);
-        const double zex = c.zexc0 * exp(-118348.0 / T) / (1.0 + pw);
+        const double pw = sqT * 3.1622776601683794e-3, ipw = 1.0 / (1.0 + pw);          // sqrt(T / 1e5)
+        const double zex = c.zexc0 * exp(-118348.0 * invT) * ipw;
         r.zxy = zex + zci;
-        r.zxy_t = zex * (118348.0 / T - 0.5 * pw / (1.0 + pw)) + zci_t;
+        r.zxy_t = zex * (118348.0 * invT - 0.5 * pw * ipw) + zci_t;
     }
 }
 
@@ -81,7 +83,7 @@ __device__ __noinline__ int chemistry_f64(double &N, double &gx, double &gy, dou
     else if (c.clump_model == 2) CR = c.clump_k0 * pow(nH, c.clump_k1);
     CR = fmax(CR, 1.0);
     const double CI = c.ci_k0 > 0.0 ? fmax(c.ci_k0 * pow(nH, c.ci_k1), 1.0) : 1.0;
-    const double cs_nH = c.cs * nH * CI, heat_rate = c.heat_rate_K * CI;
+    const double cs_nH = c.cs * nH * CI, heat_rate = c.heat_rate_K * CI, inv_nH = 1.0 / nH;
     double t_left = c.dt, att_tot = 1.0;
     int nsub = 0;
     while (t_left > 0.0 && nsub < c.max_sub) {
@@ -95,7 +97,7 @@ __device__ __noinline__ int chemistry_f64(double &N, double &gx, double &gy, dou
             if (ed * t_left > c.eps_sub * theta) dts = c.eps_sub * theta / ed;
         }
         const double A = cs_nH * dts, b = dts * r.beta * ne, rr = dts * r.alpha * CR * ne, L = 1.0 + b + rr;
-        double P = N / nH;
+        double P = N * inv_nH;
         if (CASE_A) P += dts * r.d_alpha * CR * ne * x;
         const double R0 = rr * x - b * y, onepAy = 1.0 + A * y;
         const double a2 = L * A, a1 = L * onepAy + A * (P - R0), a0 = P * A * y - R0 * onepAy;

@@ -33,9 +33,6 @@ namespace aton {
 #ifndef ATON_V4_WARPS
 #define ATON_V4_WARPS 4
 #endif
-#ifndef ATON_V4_YSHFL
-#define ATON_V4_YSHFL 1   // y neighbour terms by warp shuffles (no shared-memory patch, no __syncwarp): A/B in profiles/r02_c_step_v4.md
-#endif
 // WXQ = quads per tile row: 8 -> a 32 x 4 tile (the default), 16 -> 64 x 2
 template <int WXQ>
 struct V4Cfg {
@@ -45,7 +42,7 @@ struct V4Cfg {
     static constexpr int RAW_BUF = 4 * RAW_FIELD;        // [field][slot][RS]
     static constexpr int W_COMP = WY * WX;               // plus: slot r = (U+F_y) of row r-1; minus: slot r = row r+1
     static constexpr int W_SIGN = 4 * W_COMP;            // [comp][slot][WX]
-    static constexpr int WARP_FLOATS = 2 * RAW_BUF + (ATON_V4_YSHFL ? 0 : 2 * W_SIGN);
+    static constexpr int WARP_FLOATS = 2 * RAW_BUF + 2 * W_SIGN;
     static constexpr int WARPS = ATON_V4_WARPS, THREADS = 32 * WARPS;
     // 47 104 B per CTA for the 32 x 4 tile: 4 CTAs fit the 196 KB shared-memory carve-out and leave 60 KB of L1 for the
     // halo re-reads.  768 B more per warp (tried: a queue of deferred cells) falls into the 228 KB carve-out, 28 KB of
@@ -105,10 +102,8 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     const int xt = blockIdx.x * C::WARPS + warp;         // x tile of this warp
     if (xt * C::WX >= g.nx) return;                      // ragged last CTA in x: warps are independent
     float *raw = smem + warp * C::WARP_FLOATS;           // [2][4][6][RS], thread-private entries
-#if !ATON_V4_YSHFL
     float *wyp = raw + 2 * C::RAW_BUF;                   // [4][4][32] plus terms
     float *wym = wyp + C::W_SIGN;                        //            minus terms
-#endif
 
     // planes [zb, ze) are advanced: the whole periodic grid (0, nz), or a slab's own planes (1, nz - 1) whose
     // ghost planes 0 and nz - 1 hold the neighbours' boundary planes (no wrap is ever taken then)
@@ -118,13 +113,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     const int rowoff = (y0 + r) * g.nx + x0 + 4 * q;     // own quad inside a plane
     // y halo row of this lane: rows 0 / 3 take the row below / above the tile (others: a harmless re-read)
     const bool hbot = r == 0, htop = r == C::WY - 1;
-#if ATON_V4_YSHFL
-    // roles swapped for the rotation shuffles: the lanes of the TOP row close the row BELOW the tile (its U + F_y goes
-    // to row 0), the lanes of row 0 the row ABOVE (its U - F_y goes to the top row)
-    const int jh = htop ? (y0 == 0 ? g.ny - 1 : y0 - 1) : (hbot ? (y0 + C::WY == g.ny ? 0 : y0 + C::WY) : y0 + r);
-#else
     const int jh = hbot ? (y0 == 0 ? g.ny - 1 : y0 - 1) : (htop ? (y0 + C::WY == g.ny ? 0 : y0 + C::WY) : y0 + r);
-#endif
     const int hoff = jh * g.nx + x0 + 4 * q;
     const int hslot = hbot ? 0 : (htop ? C::WY + 1 : r + 1);
     // x halo cell of this lane: q = 0 the cell left of the tile, q = 7 the cell right of it
@@ -213,52 +202,6 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
             }
         }
         Quad t;
-#if ATON_V4_YSHFL
-        // ---- start plane m from its own state and the +z term carried from plane m-1
-#pragma unroll
-        for (int p = 0; p < 2; p++)
-#pragma unroll
-            for (int v = 0; v < 4; v++) t.v[p][v] = fma2(u.v[p][v], c.keep, zup.v[p][v]);
-        if (INPL) {
-            // ---- y: every lane sends (U + F_y) of its row to the row above and (U - F_y) to the row below by rotation
-            //      shuffles; the top-row lanes send the closed row below the tile instead (it reaches row 0), the row-0
-            //      lanes the closed row above the tile (it reaches the top row)
-            const float4 hn4 = *reinterpret_cast<const float4 *>(buf + myh);
-            const float4 hgx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + myh);
-            const float4 hgy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + myh);
-            const float4 hgz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + myh);
-            const int from_below = (lane + 32 - WXQ) & 31, from_above = (lane + WXQ) & 31;
-            const f2 sg = splat(htop ? 1.0f : -1.0f);
-#pragma unroll
-            for (int p = 0; p < 2; p++) {
-                f2 F[4], e[4] = {ld_pair(hn4, p), ld_pair(hgx4, p), ld_pair(hgy4, p), ld_pair(hgz4, p)}, ea, es, Fh[4];
-                flux_row(1, u.v[p], a[p], s[p], F);
-                closure2(e[0], e[1], e[2], e[3], ea, es);
-                flux_row(1, e, ea, es, Fh);
-#pragma unroll
-                for (int v = 0; v < 4; v++) {
-                    const f2 w = fma2(Fh[v], sg, e[v]);
-                    const f2 P = u.v[p][v] + F[v], M = u.v[p][v] - F[v];
-                    const float sp0 = htop ? lo(w) : lo(P), sp1 = htop ? hi(w) : hi(P);
-                    const float sm0 = hbot ? lo(w) : lo(M), sm1 = hbot ? hi(w) : hi(M);
-                    const f2 yp = pk(__shfl_sync(0xffffffffu, sp0, from_below), __shfl_sync(0xffffffffu, sp1, from_below));
-                    const f2 ym = pk(__shfl_sync(0xffffffffu, sm0, from_above), __shfl_sync(0xffffffffu, sm1, from_above));
-                    t.v[p][v] = fma2(yp + ym, c.h, t.v[p][v]);
-                }
-            }
-        }
-        // ---- z: complete plane m-1, seed plane m+1
-#pragma unroll
-        for (int p = 0; p < 2; p++) {
-            f2 F[4];
-            flux_row(2, u.v[p], a[p], s[p], F);
-#pragma unroll
-            for (int v = 0; v < 4; v++) {
-                pend.v[p][v] = fma2(u.v[p][v] - F[v], c.h, pend.v[p][v]);
-                zup.v[p][v] = (u.v[p][v] + F[v]) * c.h;
-            }
-        }
-#else
         if (INPL) {
             __syncwarp();                                // every lane has consumed the previous plane's y terms
             // ---- y: publish (U + F_y) for the row above, (U - F_y) for the row below
@@ -328,7 +271,6 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
                 zup.v[p][v] = (u.v[p][v] + F[v]) * c.h;
             }
         }
-#endif
         // ---- x: (U + F_x) of the cell to the left, (U - F_x) of the cell to the right
         if (INPL) {
             f2 Wp[2][4], Wm[2][4];
@@ -392,9 +334,6 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
 #undef ATON_ST4
             if (nib) atomicOr(f.defer_mask + ((unsigned)oprev >> 5), nib << (oprev & 31));
         }
-#if ATON_V4_YSHFL
-        pend = t;
-#else
         // ---- y terms of plane m, written straight into the carried registers
         if (INPL) {
             const int rp = r * C::WX + 4 * q;
@@ -409,7 +348,6 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         } else {
             pend = t;
         }
-#endif
         oprev = ocur;
         kcur = kcur + 1 == g.nz ? 0 : kcur + 1;
         ocur = kcur * plane + rowoff;

@@ -73,26 +73,48 @@ def combine_sums(local: List[float], group=None, world: int = 1) -> List[float]:
 
 
 class SlabAton:
-    """One rank's slab of a global nx x ny x nz box.  `fields` are this rank's planes (nz_local, ny, nx)."""
+    """One rank's slab of a global nx x ny x nz box.  `fields` are this rank's planes (nz_local, ny, nx).
+
+    Two ways to move the halos, same results:
+      native=True   the library's own NCCL communicator (aton_comm_init; rank 0's unique id is broadcast through the
+                    torch.distributed group) and aton_step_slab: the whole run of steps is one C call, the exchange runs
+                    on a second stream beside the interior planes;
+      native=False  aton_halo_pack -> exchange_halos (torch.distributed P2P: gloo on CPU tensors in the tests, NCCL on
+                    GPUs) -> aton_halo_unpack -> aton_step(dt, 1), one step at a time."""
 
     def __init__(self, nx: int, ny: int, nz: int, lx_cm: float, params: Dict[str, float], rank: int = 0,
-                 world: int = 1, group=None, stream: Optional[torch.cuda.Stream] = None):
-        self.rank, self.world, self.group = rank, world, group
+                 world: int = 1, group=None, stream: Optional[torch.cuda.Stream] = None, native: bool = False):
+        self.rank, self.world, self.group, self.native = rank, world, group, native
         self.z_begin, self.nz_local = slab_range(nz, world, rank)
         self.params = dict(params)
         self.ctx = aton.Aton(nx, ny, nz, lx_cm, params, stream, slab=(self.z_begin, self.nz_local))
-        self.buf = {k: torch.empty((4, ny, nx), dtype=torch.float32, device="cuda")
-                    for k in ("send_lo", "send_hi", "recv_lo", "recv_hi")}
+        self.buf = None
+        if native:
+            comm_id = None
+            if world > 1:
+                box = [aton.comm_unique_id() if rank == 0 else None]
+                dist.broadcast_object_list(box, src=0, group=group)
+                comm_id = box[0]
+            self.ctx.comm_init(comm_id, rank, world)
+        else:
+            self.buf = {k: torch.empty((4, ny, nx), dtype=torch.float32, device="cuda")
+                        for k in ("send_lo", "send_hi", "recv_lo", "recv_hi")}
 
     def set_fields(self, nH, x, T, N=None, Fx=None, Fy=None, Fz=None):
         self.ctx.set_fields(nH, x, T, N, Fx, Fy, Fz)
-        # <n_H> of the linear clumping law is a GLOBAL mean: all-reduce the library's own sums, hand them back
-        self.ctx.set_mean_from_sums(combine_sums(self.ctx.reduce_sums(), self.group, self.world))
+        # <n_H> of the linear clumping law is a GLOBAL mean
+        if self.native:
+            self.ctx.sync_mean_density()
+        else:       # all-reduce the library's own sums, hand them back
+            self.ctx.set_mean_from_sums(combine_sums(self.ctx.reduce_sums(), self.group, self.world))
 
     def set_sources(self, pos, rate):
         self.ctx.set_sources(pos, rate)          # global positions; the library keeps this slab's sources
 
     def step(self, dt: float, n_steps: int = 1):
+        if self.native:
+            self.ctx.step_slab(dt, n_steps)
+            return
         b = self.buf
         for _ in range(n_steps):
             self.ctx.halo_pack(b["send_lo"], b["send_hi"])
@@ -104,7 +126,9 @@ class SlabAton:
         return self.ctx.get_fields(**kw)
 
     def reduce(self) -> Dict[str, float]:
-        """Global diagnostics: the slabs' raw sums all-reduced, the means formed by the library."""
+        """Global diagnostics: the slabs' raw sums combined, the means formed by the library."""
+        if self.native:
+            return self.ctx.reduce_global()
         return self.ctx.diag_from_sums(combine_sums(self.ctx.reduce_sums(), self.group, self.world))
 
     def close(self):

@@ -110,6 +110,32 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
         assert max(err.values()) <= TOL_1STEP, (kw, err)
 
 
+@pytest.mark.parametrize("case", ["cfg1_32", "cfg3_twin64", "cfg4_twin64", "cfg3_twin40"])
+def test_hll_flux_against_oracle(orc, case):
+    """SURVEY NEXT-3 / PAPER.md:L85: the HLL intercell flux (aton_params_t.flux = 1) against the oracle's
+    orc_transport_hll, same bars as the Lax-Friedrichs path: 1e-4 after one step from the oracle's warm HLL state,
+    relative L1 1e-3 after the run; and the run differs from the LF run (it is another scheme, less diffusive)."""
+    build, k, n_steps = _cases()[case]
+    n_steps = min(n_steps, 150)
+    w = build()
+    w.params.update(flux=1)
+    ww = _warm(orc, w, k)
+    st, p = _oracle_cached(orc, ww, 1)
+    assert p.flux == 1
+    g, diag = gpu_run(ww, 1)
+    err = max_rel_errors(g, st, p.c)
+    assert diag["n_nonfinite"] == 0 and max(err.values()) <= TOL_1STEP, (case, err)
+    st, p = _oracle_cached(orc, w, n_steps)
+    g, diag = gpu_run(w, n_steps)
+    err = l1_errors(g, st, p.c)
+    assert diag["n_nonfinite"] == 0 and diag["steps_done"] == n_steps
+    assert err["x_vol"] <= TOL_XVOL and max(err[f] for f in ("N", "F", "F_rel", "x", "T")) <= TOL_L1, (case, err)
+    assert diag["f_max"] <= 1.0 + 1e-5 and diag["N_min"] >= 0.0
+    w.params.update(flux=0)
+    g0, _ = gpu_run(w, n_steps)
+    assert np.abs(g0["N"] - g["N"]).sum() > 1e-2 * np.abs(g["N"]).sum()
+
+
 @pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 def test_reduce_matches_oracle(orc, variant):
     w = wl.synthetic_warm_state(twin(4, 32, 10))

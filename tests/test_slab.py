@@ -147,20 +147,65 @@ def test_slab_class_world_size_1_and_errors():
     full.set_fields(nH, x0, T0); full.set_sources(pos, rate); full.step(dt, 9)
     ref, dref = full.get_fields(device="cuda"), full.reduce()
     full.close()
-    s = slab.SlabAton(nx, ny, nz, dx * nx, p)              # world 1: a rank that is its own neighbour
-    s.set_fields(nH, x0, T0); s.set_sources(pos, rate); s.step(dt, 9)
-    out, d = s.get_fields(device="cuda"), s.reduce()
-    for k in ref:
-        assert torch.equal(out[k], ref[k]), k
-    assert d["x_vol"] == pytest.approx(dref["x_vol"], rel=1e-12) and d["gamma_vol"] == pytest.approx(dref["gamma_vol"], rel=1e-6)
-    with pytest.raises(aton.AtonError):
-        s.ctx.step(dt, 2)                                  # one step per halo exchange
-    s.close()
+    for native in (False, True):                           # world 1: a rank that is its own neighbour
+        s = slab.SlabAton(nx, ny, nz, dx * nx, p, native=native)
+        s.set_fields(nH, x0, T0); s.set_sources(pos, rate)
+        if native:
+            s.step(dt, 4); s.step(dt, 5)                   # aton_step_slab: runs of steps, ghost planes carried over
+        else:
+            s.step(dt, 9)
+        out, d = s.get_fields(device="cuda"), s.reduce()
+        for k in ref:
+            assert torch.equal(out[k], ref[k]), (native, k)
+        assert d["x_vol"] == pytest.approx(dref["x_vol"], rel=1e-12) and d["gamma_vol"] == pytest.approx(dref["gamma_vol"], rel=1e-6)
+        assert d["steps_done"] == 9 and d["subcycles_total"] == dref["subcycles_total"]
+        with pytest.raises(aton.AtonError):
+            s.ctx.step(dt, 2)                              # aton_step: one step per halo exchange
+        if not native:
+            with pytest.raises(aton.AtonError):
+                s.ctx.step_slab(dt, 1)                     # aton_step_slab needs aton_comm_init
+        s.close()
     with pytest.raises(aton.AtonError):
         aton.Aton(24, 8, 6, dx * 24, p, slab=(0, 3))       # variant 4 needs nx % 32 == 0
+    hp = dict(p); hp.update(flux=1)
+    with pytest.raises(aton.AtonError):
+        aton.Aton(32, 8, 6, dx * 32, hp, slab=(0, 3))      # the HLL kernel runs on undivided grids only
     with pytest.raises(aton.AtonError):
         aton.Aton(32, 8, 6, dx * 32, p, slab=(4, 3))       # planes outside the grid
     a = aton.Aton(32, 8, 6, dx * 32, p)
     with pytest.raises(aton.AtonError):
         a.halo_pack(torch.zeros(4, 8, 32, device="cuda"), torch.zeros(4, 8, 32, device="cuda"))   # not a slab
     a.close()
+
+
+@pytest.mark.gpu
+def test_native_slab_step_with_nccl_self_exchange_against_the_oracle(orc):
+    """aton_step_slab through a real NCCL communicator (one rank: every send pairs with the rank's own receive, the same
+    code path as N ranks) on a grid with several z planes per launch range, against the ORACLE (not only the undivided
+    CUDA run): relative L1 <= 1e-3 after 30 steps, and bit-identical to the undivided CUDA run."""
+    from paper_1004_2503_b200 import aton
+    from parity_util import l1_errors
+    nx, ny, nz = 64, 16, 10
+    nH, p, dx, pos, rate = _case(nx, ny, nz, seed=9)
+    x0, T0 = torch.full_like(nH, 1e-3), torch.full_like(nH, 100.0)
+    dt, steps = wl.courant_dt(dx), 30
+    full = aton.Aton(nx, ny, nz, dx * nx, p)
+    full.set_fields(nH, x0, T0); full.set_sources(pos, rate); full.step(dt, steps)
+    ref = full.get_fields(device="cuda")
+    full.close()
+    s = slab.SlabAton(nx, ny, nz, dx * nx, p, native=False)
+    s.ctx.comm_init(aton.comm_unique_id(), 0, 1)           # a 1-rank NCCL communicator instead of the copy shortcut
+    s.native = True
+    s.set_fields(nH, x0, T0); s.set_sources(pos, rate)
+    s.step(dt, steps)
+    out, d = s.get_fields(device="cpu"), s.reduce()
+    s.close()
+    for k in ref:
+        assert torch.equal(out[k], ref[k].cpu()), k
+    zero = np.zeros((nz, ny, nx), np.float32)
+    st = orc.State(nH.cpu().numpy(), x0.cpu().numpy(), T0.cpu().numpy(), zero, zero, zero, zero)
+    op = orc.make_params(p, dx, float(nH.double().mean()))
+    orc.step(st, op, dt, steps, pos.double().numpy(), rate.numpy())
+    err = l1_errors({k: v.numpy() for k, v in out.items()}, st, op.c)
+    assert max(err[k] for k in ("N", "F", "x", "T")) <= 1e-3 and err["x_vol"] <= 1e-3, err
+    assert d["x_vol"] == pytest.approx(st.x.mean(), abs=1e-3) and d["n_nonfinite"] == 0
