@@ -205,6 +205,46 @@ int aton_step_slab(aton_t *ctx, double dt, int n_steps);
 int aton_reduce_global(aton_t *ctx, aton_diag_t *out);
 int aton_sync_mean_density(aton_t *ctx);
 
+/* ---- analysis and source front end around the step (nothing here runs per step) ---- */
+
+/* Clumping-factor measurement (section 3.2.1): over every block x block x block cells of the current
+ * state (the paper: 8^3 cells of its fine run = one cell of its coarse run),
+ *   C_R = <n_H^2 x^2> / <n_H x>^2,   C_I = <N (1-x) n_H> / (<N> <(1-x) n_H>)      (L247),
+ * with the block's mean density <n_H> and its ionised fraction <n_H x>/<n_H> (the two variables the paper bins C against,
+ * Fig.12-13).  A factor whose denominator vanishes is 1.  Each output is [nz/block][ny/block][nx/block] float32, host or
+ * device as said by on_device; block must divide nx, ny and nz.  Undivided contexts only.  Synchronises. */
+int aton_clumping_blocks(aton_t *ctx, int block, float *nH_mean, float *x_mean, float *C_R, float *C_I, int on_device);
+
+/* 2-D distribution of two per-cell quantities of the current state (the Gamma(n_H), x(n_H), (1-x)(n_H) planes of PAPER.md
+ * Fig.5-19; L417).  A value v lands in bin floor((f(v) - lo)/(hi - lo) * nbins) of its axis, f = log10 on a log axis;
+ * values outside [lo, hi) (or <= 0 on a log axis) are tallied in *outside.  counts is [nb][na] int64 (counts[ib*na + ia]),
+ * host or device as said by on_device; na * nb <= 4096.  Integer counts: deterministic.  Synchronises. */
+#define ATON_Q_NH 0       /* n_H [cm^-3] */
+#define ATON_Q_X 1        /* ionised fraction x */
+#define ATON_Q_NEUTRAL 2  /* 1 - x */
+#define ATON_Q_T 3        /* T [K] */
+#define ATON_Q_N 4        /* photon density N [cm^-3] */
+#define ATON_Q_GAMMA 5    /* photo-ionisation rate c sigma_n N [1/s] (Eq.15) */
+int aton_histogram2d(aton_t *ctx, int quantity_a, int quantity_b, int log_a, int log_b, double a_lo, double a_hi,
+                     double b_lo, double b_hi, int na, int nb, long long *counts, long long *outside, int on_device);
+
+/* Source front end (section 2.3): the star particles of snapshot p+1 -> emission rates for the transfer
+ * from t_p to t_p1 [s, ages of the Universe], then aton_set_sources.  Per particle: pos (box units), age at t_p1 [s],
+ * lifetime L as an ionising source [s] (the paper draws it between 5 and 20 Myr: the draw is the caller's), n_baryons;
+ * Ndot = photons_per_baryon * n_baryons / L (the paper: 24 000 - 98 000 photons per stellar baryon).  With
+ * a_p = age - (t_p1 - t_p): a_p > L discarded; a_p < 0 (born in the interval) the diluted rate min(age, L)/(t_p1 - t_p) Ndot;
+ * otherwise min(1, (L - a_p)/(t_p1 - t_p)) Ndot -- each branch emits exactly the photons the star emits in the interval.
+ * Then Eq.8-9: Ndot_eff = Ndot f_esc B, B = max(1, a_b exp(k_b / t)) at the middle of the interval (k_b in s; Table 1;
+ * DESIGN.md readings G5, G6).  Arrays are host or device as said by on_device.  Synchronises. */
+int aton_set_star_sources(aton_t *ctx, long long n, const float *pos, const double *age, const double *lifetime,
+                          const double *nbaryons, double photons_per_baryon, double t_p, double t_p1, double f_esc,
+                          double a_b, double k_b, int on_device);
+
+/* Thomson optical depth, Eq.10: tau = c sigma_T int n_e dt for a history x(z) of the mass-weighted
+ * ionised fraction (n points, z ascending, HOST arrays) in flat LCDM: n_e = x nH0 (1+z)^3, H = H0 sqrt(Om (1+z)^3 + 1 - Om)
+ * [H0 in 1/s, nH0 in cm^-3]; trapezoid rule.  Synchronises. */
+int aton_thomson_tau(aton_t *ctx, long long n, const double *z, const double *x, double nH0, double H0, double Om, double *tau);
+
 void aton_free(aton_t *ctx);
 
 /* Message of the last failing call on ctx (ctx-owned), or of the last failing aton_init if ctx is

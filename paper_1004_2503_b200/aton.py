@@ -21,7 +21,9 @@ EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt"
            "aton_get_fields", "aton_reduce", "aton_set_kernel", "aton_launch_count", "aton_set_timing",
            "aton_kernel_time", "aton_fixup_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
            "aton_reduce_sums", "aton_diag_from_sums", "aton_set_mean_from_sums", "aton_comm_unique_id", "aton_comm_init",
-           "aton_step_slab", "aton_reduce_global", "aton_sync_mean_density", "aton_free", "aton_last_error")
+           "aton_step_slab", "aton_reduce_global", "aton_sync_mean_density", "aton_clumping_blocks", "aton_histogram2d",
+           "aton_set_star_sources", "aton_thomson_tau", "aton_free", "aton_last_error")
+Q_NH, Q_X, Q_NEUTRAL, Q_T, Q_N, Q_GAMMA = range(6)
 COMM_ID_BYTES = 128
 NSUMS = 15
 
@@ -119,6 +121,14 @@ def load_library(path: Optional[str] = None):
     L.aton_reduce_global.argtypes = [vp, C.POINTER(Diag)]
     L.aton_sync_mean_density.restype = C.c_int
     L.aton_sync_mean_density.argtypes = [vp]
+    L.aton_clumping_blocks.restype = C.c_int
+    L.aton_clumping_blocks.argtypes = [vp, C.c_int, fp, fp, fp, fp, C.c_int]
+    L.aton_histogram2d.restype = C.c_int
+    L.aton_histogram2d.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int] + [C.c_double] * 4 + [C.c_int, C.c_int, vp, vp, C.c_int]
+    L.aton_set_star_sources.restype = C.c_int
+    L.aton_set_star_sources.argtypes = [vp, C.c_longlong, fp, dp, dp, dp] + [C.c_double] * 6 + [C.c_int]
+    L.aton_thomson_tau.restype = C.c_int
+    L.aton_thomson_tau.argtypes = [vp, C.c_longlong, dp, dp, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]
     L.aton_free.restype = None
     L.aton_free.argtypes = [vp]
     L.aton_last_error.restype = C.c_char_p
@@ -267,6 +277,41 @@ class Aton:
 
     def sync_mean_density(self):
         self._check(self._L.aton_sync_mean_density(self._h))
+
+    def clumping_blocks(self, block: int = 8, device="cuda") -> Dict[str, torch.Tensor]:
+        """aton_clumping_blocks: dict of [nz/b, ny/b, nx/b] float32 tensors nH, x, C_R, C_I."""
+        nz, ny, nx = self.shape
+        shape = (nz // block, ny // block, nx // block)
+        dev = torch.device(device)
+        out = {k: torch.empty(shape, dtype=torch.float32, device=dev) for k in ("nH", "x", "C_R", "C_I")}
+        n = shape[0] * shape[1] * shape[2]
+        self._check(self._L.aton_clumping_blocks(self._h, int(block), *[_ptr(out[k], n, torch.float32, dev.type == "cuda")
+                                                                          for k in ("nH", "x", "C_R", "C_I")], int(dev.type == "cuda")))
+        return out
+
+    def histogram2d(self, qa: int, qb: int, log_a: bool, log_b: bool, a_range, b_range, na: int, nb: int):
+        """aton_histogram2d: (counts[nb, na] int64 CPU tensor, number of cells outside the ranges)."""
+        counts = torch.zeros((nb, na), dtype=torch.int64)
+        outside = C.c_longlong(0)
+        self._check(self._L.aton_histogram2d(self._h, qa, qb, int(log_a), int(log_b), float(a_range[0]), float(a_range[1]),
+                                             float(b_range[0]), float(b_range[1]), na, nb, C.c_void_p(counts.data_ptr()),
+                                             C.cast(C.byref(outside), C.c_void_p), 0))
+        return counts, int(outside.value)
+
+    def set_star_sources(self, pos, age, lifetime, nbaryons, photons_per_baryon, t_p, t_p1, f_esc, a_b, k_b):
+        n = age.numel()
+        dev = pos.is_cuda
+        self._check(self._L.aton_set_star_sources(self._h, n, _ptr(pos, 3 * n, torch.float32, dev),
+                                                  *[_ptr(t, n, torch.float64, dev) for t in (age, lifetime, nbaryons)],
+                                                  float(photons_per_baryon), float(t_p), float(t_p1), float(f_esc), float(a_b),
+                                                  float(k_b), int(dev)))
+
+    def thomson_tau(self, z: torch.Tensor, x: torch.Tensor, nH0: float, H0: float, Om: float) -> float:
+        n = z.numel()
+        tau = C.c_double()
+        self._check(self._L.aton_thomson_tau(self._h, n, _ptr(z, n, torch.float64, False), _ptr(x, n, torch.float64, False),
+                                             float(nH0), float(H0), float(Om), C.byref(tau)))
+        return tau.value
 
     def set_timing(self, on: bool):
         self._check(self._L.aton_set_timing(self._h, int(bool(on))))

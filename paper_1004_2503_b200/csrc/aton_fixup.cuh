@@ -74,9 +74,15 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
     // redo the queued cells (all threads of the block call this together)
     auto drain = [&]() {
         const int n = qn;
-        // self-scheduling: a lane takes the next cell when it is done with its own, so a round lasts as long as its
-        // slowest cell, not as long as the slowest cell of every stride (source cells take tens of sub-cycles)
-        for (int it = atomicAdd(&qhead, 1); it < n; it = atomicAdd(&qhead, 1)) {
+        // self-scheduling by warps: a warp takes the next 32 cells when it is done with its own, so a round lasts as
+        // long as its slowest warp, not as long as the slowest cell of every stride (source cells take tens of
+        // sub-cycles); one shared-memory atomic per 32 cells
+        for (;;) {
+            int it = 0;
+            if ((threadIdx.x & 31) == 0) it = atomicAdd(&qhead, 32);
+            it = __shfl_sync(0xffffffffu, it, 0) + (threadIdx.x & 31);
+            if (it - (int)(threadIdx.x & 31) >= n) break;
+            if (it >= n) continue;
             const int id = queue[it];
             float N = f.N1[id], gx = f.Gx1[id], gy = f.Gy1[id], gz = f.Gz1[id];
             float x = f.x[id], T = f.T[id];

@@ -30,7 +30,7 @@ def lib():
 def _declared_functions():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(aton_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(aton_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -43,7 +43,7 @@ def test_library_exports_every_declared_symbol(lib):
     assert sorted(aton.EXPORTS) == names
     # the dynamic symbol table holds them as plain C names (no mangling)
     out = subprocess.check_output(["nm", "-D", "--defined-only", aton.LIB_PATH], text=True)
-    exported = set(re.findall(r"\bT (aton_[a-z_]+)$", out, flags=re.M))
+    exported = set(re.findall(r"\bT (aton_[a-z0-9_]+)$", out, flags=re.M))
     assert set(names) <= exported
 
 
