@@ -222,6 +222,10 @@ int check_dt(aton_ctx *ctx, double *dt, const char *who) {
 // read from global memory: rewritten (stream-ordered, no host synchronisation) only when something they hold changed.
 cudaError_t prepare_step(aton_ctx *ctx, double dt) {
     if (!ctx->fix_dirty && ctx->fix_dt == dt) return cudaSuccess;
+    if (ctx->step_graph) {             // the captured pair of steps holds the old constants
+        cudaGraphExecDestroy(ctx->step_graph);
+        ctx->step_graph = nullptr;
+    }
     ctx->sc = make_step_const(ctx, dt);
     ctx->scd = make_step_const_d(ctx, dt);
     FixArgs a[2];
@@ -349,8 +353,8 @@ static int init_common(aton_t **out, const aton_grid_t *grid, const aton_box_t *
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->defer_mask, 0, defer_bytes, ctx->stream);
     ctx->stiff_cap = (unsigned)std::max<size_t>(ctx->nalloc / 16, 4096);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stiff_q, sizeof(int) * (size_t)ctx->stiff_cap);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stiff_n, 2 * sizeof(unsigned));
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stiff_n, 0, 2 * sizeof(unsigned), ctx->stream);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->stiff_n, 4 * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->stiff_n, 0, 4 * sizeof(unsigned), ctx->stream);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->fixargs, 2 * sizeof(FixArgs));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->src_bits, defer_bytes);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->src_bits, 0, defer_bytes, ctx->stream);
@@ -381,6 +385,7 @@ void aton_free(aton_t *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     slab_comm_free(ctx);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_fix) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_stiff) cudaEventDestroy(e);
@@ -487,7 +492,7 @@ int aton_set_fields(aton_t *ctx, const float *nH, const float *x, const float *T
         return fail(ctx, ATON_EINVAL, "aton_set_fields: n_H must be finite and > 0 everywhere (min %g)", red[R_NHMIN]);
     if (!ctx->mean_set) ctx->nH_mean = red[R_M] / (double)ctx->ncell;
     ctx->fix_dirty = true;
-    CU(ctx, cudaMemsetAsync(ctx->stiff_n, 0, 2 * sizeof(unsigned), ctx->stream));
+    CU(ctx, cudaMemsetAsync(ctx->stiff_n, 0, 4 * sizeof(unsigned), ctx->stream));
     ctx->steps_done = 0;
     ctx->fast_subcycles = 0;
     ctx->time_s = 0.0;
@@ -584,8 +589,50 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     if (ctx->slab && n_steps > 1)
         return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first, or use aton_step_slab)");
     if (n_steps > 0) CU(ctx, prepare_step(ctx, dt));
-    for (int s = 0; s < n_steps; s++) {
-        CU(ctx, launch_step_planes(ctx, ctx->slab ? 1 : 0, ctx->slab ? ctx->nz_local + 1 : ctx->g.nz));
+    const int zb = ctx->slab ? 1 : 0, ze = ctx->slab ? ctx->nz_local + 1 : ctx->g.nz;
+    int s = 0;
+    // Small grids (configs 1-2) are launch bound: three launches per step, each a few microseconds of work (SURVEY
+    // 3(iii), H7).  Capture one ping-pong pair of steps in a CUDA graph once and replay it.
+    if (!ctx->slab && !ctx->timing && !ctx->graph_failed && ctx->ncell <= ((size_t)1 << 22) && n_steps >= 4) {
+        if (ctx->cur == 1) {           // the captured pair starts from buffer 0
+            CU(ctx, launch_step_planes(ctx, zb, ze));
+            ctx->cur = 0; ctx->steps_done++; ctx->time_s += dt; s++;
+        }
+        if (!ctx->step_graph) {
+            const long long l0 = ctx->launches, f0 = ctx->fast_subcycles;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                e = launch_step_planes(ctx, zb, ze);
+                ctx->cur = 1;
+                if (e == cudaSuccess) e = launch_step_planes(ctx, zb, ze);
+                ctx->cur = 0;
+                const cudaError_t e2 = cudaStreamEndCapture(ctx->stream, &graph);
+                if (e == cudaSuccess) e = e2;
+            }
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&ctx->step_graph, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+            ctx->graph_launches = ctx->launches - l0;
+            ctx->graph_fast = ctx->fast_subcycles - f0;
+            ctx->launches = l0;            // capturing launched nothing
+            ctx->fast_subcycles = f0;
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                ctx->step_graph = nullptr;
+                ctx->graph_failed = true;
+            }
+        }
+        while (ctx->step_graph && n_steps - s >= 2) {
+            CU(ctx, cudaGraphLaunch(ctx->step_graph, ctx->stream));
+            ctx->launches += ctx->graph_launches;
+            ctx->fast_subcycles += ctx->graph_fast;
+            ctx->steps_done += 2;
+            ctx->time_s += 2 * dt;
+            s += 2;
+        }
+    }
+    for (; s < n_steps; s++) {
+        CU(ctx, launch_step_planes(ctx, zb, ze));
         ctx->cur = 1 - ctx->cur;
         ctx->steps_done++;
         ctx->time_s += dt;

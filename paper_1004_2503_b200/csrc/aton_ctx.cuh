@@ -62,6 +62,9 @@ struct aton_ctx {
     std::vector<cudaEvent_t> ev_stiff;     // ... and for step_stiff_kernel
     aton::StepConst sc{};                  // constants of the step size fix_dt (prepare_step)
     aton::StepConstD scd{};
+    cudaGraphExec_t step_graph = nullptr;  // two steps (one ping-pong pair) captured once for small, launch-bound grids
+    bool graph_failed = false;             // capture or instantiation failed once: plain launches from then on
+    long long graph_launches = 0, graph_fast = 0;   // what one replay adds to `launches` / `fast_subcycles`
     aton::SlabComm *comm = nullptr;        // aton_comm_init (slab contexts only)
     bool halo_valid = false;               // the ghost planes of the current buffer hold the neighbours' boundary planes
     char err[512] = "";

@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(128) step_stiff_kernel(const FixArgs *fa) {
 constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS, FIXUP_GROUP = 8;
 
 template <int FLAGS>
-__global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
+__global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
     __shared__ int queue[FIXUP_QCAP];
     __shared__ int qn, qhead;
     const FieldsIO &f = fa->f;
@@ -98,16 +98,15 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
                 const unsigned slot = atomicAdd(f.stiff_n, 1u);
                 if (slot < f.stiff_cap) {
                     f.stiff_q[slot] = id;
-                } else {                    // queue full (the cap is ncell / 16): redo it here
-                    double Nd = (double)f.N1[id] + ((f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) ? source_lookup_d(f, id, fa->cd.dt) : 0.0);
-                    double ax = f.Gx1[id], ay = f.Gy1[id], az = f.Gz1[id], xd = f.x[id], Td = f.T[id];
-                    const int nd = chemistry_f64<FLAGS>(Nd, ax, ay, az, xd, Td, (double)__ldg(f.nH + id), fa->cd);
-                    f.N1[id] = (float)Nd; f.Gx1[id] = (float)ax; f.Gy1[id] = (float)ay; f.Gz1[id] = (float)az;
-                    f.x[id] = (float)xd; f.T[id] = (float)Td;
-                    nsub_extra += nd - 1;
-                    nsub_max = max(nsub_max, nd);
+                } else {                    // queue full (more than ncell / 16 stiff cells): this one stays fp32
+                    N = f.N1[id]; gx = f.Gx1[id]; gy = f.Gy1[id]; gz = f.Gz1[id]; x = f.x[id]; T = f.T[id];
+                    if (f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) N += source_lookup(f, id, fa->c.dt);
+                    const int n32 = chemistry<FLAGS, false>(N, gx, gy, gz, x, T, __ldg(f.nH + id), fa->c);
+                    f.N1[id] = N; f.Gx1[id] = gx; f.Gy1[id] = gy; f.Gz1[id] = gz;
+                    f.x[id] = x; f.T[id] = T;
+                    nsub_extra += n32 - 1;
+                    nsub_max = max(nsub_max, n32);
                     ncell++;
-                    atomicAdd(f.stats + 3, 1ull);
                 }
             }
         }
@@ -119,7 +118,15 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
     // once and an empty group (almost all of them away from fronts and sources) costs one block-wide vote
     const int end = word0 + nwords;
     const int ngroups = (nwords + FIXUP_GROUP * FIXUP_THREADS - 1) / (FIXUP_GROUP * FIXUP_THREADS);
-    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    // groups are handed out by a global cursor (f.stiff_n[2]): sources and fronts cluster, a static split leaves some
+    // blocks with several times the cells of others
+    __shared__ int s_grp;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_grp = (int)atomicAdd(f.stiff_n + 2, 1u);
+        __syncthreads();
+        const int grp = s_grp;
+        if (grp >= ngroups) break;
         unsigned bits[FIXUP_GROUP];
         unsigned any = 0u;
 #pragma unroll
@@ -128,7 +135,7 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
             bits[k] = w < end ? f.defer_mask[w] : 0u;
             any |= bits[k];
         }
-        if (!__syncthreads_or(any != 0u)) continue;
+        if (!__syncthreads_or(any != 0u)) continue;       // (the barrier at the loop top orders s_grp's next write)
 #pragma unroll
         for (int k = 0; k < FIXUP_GROUP; k++) {
             if (bits[k]) {
@@ -158,6 +165,12 @@ __global__ void __launch_bounds__(FIXUP_THREADS) step_fixup_kernel(const FixArgs
         atomicAdd(f.stats, (unsigned long long)nsub_extra);
         atomicMax(f.stats + 1, (unsigned long long)nsub_max);
         atomicAdd(f.stats + 2, (unsigned long long)ncell);
+    }
+    // the last block to finish re-arms the group cursor ([3] counts finished blocks)
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(f.stiff_n + 3, 1u) == gridDim.x - 1) { f.stiff_n[2] = 0u; f.stiff_n[3] = 0u; }
     }
 }
 

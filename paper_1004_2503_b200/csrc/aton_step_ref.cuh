@@ -26,7 +26,9 @@ struct FieldsIO {
     unsigned *defer_mask;               // variant 2: 1 bit per cell, set = needs sub-cycling (fix-up kernel clears it)
     const unsigned *src_bits;           // variant 4: 1 bit per cell, set = the cell holds a source
     int *stiff_q;                       // variant 4: [stiff_cap] ids of cells whose fp32 sub-cycling bailed out (they keep
-    unsigned *stiff_n;                  //   their transported values); [0] = ids queued this step (may exceed the cap)
+    unsigned *stiff_n;                  //   their transported values); [0] = ids queued this step (may exceed the cap),
+                                        //   [1] finished blocks of step_stiff_kernel, [2] group cursor and [3] finished
+                                        //   blocks of step_fixup_kernel
     unsigned stiff_cap;
     int fix_inject;                     // 1: the redo paths inject the sources (variant 4); 0: the step kernel did (variant 2)
 };

@@ -197,6 +197,34 @@ def test_determinism_and_checkpoint(variant):
     assert d12["x_vol"] == pytest.approx(da["x_vol"], rel=1e-6)
 
 
+@pytest.mark.parametrize("variant", [None, 0, 2], ids=VIDS)
+def test_cuda_graph_replay_equals_plain_launches(variant):
+    """Small grids replay a captured pair of steps (aton_step with n_steps >= 4); stepping one step per
+    call never captures.  Same bits, same counters, whatever the parity of the step counts and after a change of dt."""
+    from paper_1004_2503_b200 import aton
+    w = wl.make_config(1)
+    runs = []
+    for chunks in ([41], [1] * 41, [7, 1, 12, 21], [4, 37]):
+        a = aton.from_workload(w)
+        if variant is not None:
+            a.set_kernel(variant)
+        for c in chunks:
+            a.step(w.dt, c)
+        a.step(0.5 * w.dt, 9 if len(chunks) != 41 else 1)            # new dt: the captured graph must be rebuilt
+        for _ in range(8 if len(chunks) == 41 else 0):
+            a.step(0.5 * w.dt, 1)
+        runs.append(({k: v.numpy() for k, v in a.get_fields(device="cpu").items()}, a.reduce(), a.launch_count()))
+        a.close()
+    for g, d, launches in runs[1:]:
+        for k in g:
+            assert np.array_equal(g[k], runs[0][0][k]), k
+        for k in ("steps_done", "subcycles_total", "subcycles_max", "cells_subcycled", "cells_fp64"):
+            assert d[k] == runs[0][1][k], k
+        assert d["time_s"] == pytest.approx(runs[0][1]["time_s"], rel=1e-12)
+        assert launches == runs[0][2]                                # gpu_launches counts replayed kernels too
+    assert runs[0][1]["steps_done"] == 50
+
+
 @pytest.mark.parametrize("variant,tiles", [(2, ((6, 0), (14, 0), (6, 5), (6, 40), (14, 1)))], ids=["v2"])
 def test_tile_shape_independence(variant, tiles):
     """V4: the tiled kernels' result does not depend on the tile shape (bitwise)."""
