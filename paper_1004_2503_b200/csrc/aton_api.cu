@@ -54,7 +54,7 @@ StepConst make_step_const(const aton_ctx *ctx, double dt) {
     // when the fp32 sub-cycling hands a cell to the fp64 path (chemistry<.., BAIL>; thresholds measured against the
     // 1-step bar at 256^3 / 512^3 / 1024^3: profiles/r02_b_fixup.md)
     s.stiff_kappa = 1.0f / 64.0f;
-    s.stiff_sens = 1.0f;
+    s.stiff_sens = 8.0f;
     s.stiff_nsub = 1 << 30;
     return s;
 }

@@ -157,84 +157,118 @@ __device__ __forceinline__ float clumping_i(float nH, const StepConst &c) {
 // heating and cooling cancel to better than STIFF_KAPPA: the sub-step eps E/|H - Lambda| is then ill-conditioned
 // (the fp32 rate fits carry ~3e-6) and the caller redoes the cell with chemistry_f64 (aton_physics_f64.cuh).
 
+// One cell on its way through the sub-cycled operator: chem_begin, then chem_substep until it returns non-zero.
+struct ChemCell {
+    float N, x, T, y;        // y = 1 - x is carried: y' = y - delta keeps the neutral fraction's own digits (H1)
+    float nH, CR, inv_nH, cs_nH, heat_rate;
+    float t_left, att_tot, sens;
+    int nsub;
+};
+
+__device__ __forceinline__ void chem_begin(ChemCell &s, float N, float x, float T, float nH, const StepConst &c) {
+    s.N = N; s.x = x; s.T = T; s.y = 1.0f - x;
+    s.nH = nH;
+    s.CR = clumping(nH, c);
+    s.inv_nH = f_rcp(nH);
+    const bool ci_on = c.ci_k0 > 0.0f;
+    const float CI = ci_on ? clumping_i(nH, c) : 1.0f;
+    s.cs_nH = ci_on ? c.cs * nH * CI : c.cs * nH;
+    s.heat_rate = ci_on ? c.heat_rate_K * CI : c.heat_rate_K;
+    s.t_left = c.dt;
+    s.att_tot = 1.0f;
+    s.sens = 0.0f;
+    s.nsub = 0;
+}
+
+// One sub-step.  Returns 0: more to do; 1: the step is complete (s.N, s.x, s.T final, G *= s.att_tot); -1 (BAIL only): give up.
+template <int FLAGS, bool BAIL>
+__device__ __forceinline__ int chem_substep(ChemCell &s, const StepConst &c) {
+    constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL;
+    if (!(s.t_left > 0.0f) || s.nsub >= c.max_sub) return 1;
+    if (BAIL && s.nsub >= c.stiff_nsub) return -1;
+    const float N = s.N, x = s.x, T = s.T, y = s.y, nH = s.nH, CR = s.CR, t_left = s.t_left;
+    Rates r;
+    rates<FLAGS>(T, c, r);
+    const float ne = x * nH;
+    const float theta = (1.0f + x) * T;
+    float dts = t_left;
+    if (COOL) {
+        // estimated net heating rate / (1.5 kB nH)  [K/s]
+        float lamK = nH * (x * x * fmaf(CR, r.zrec, r.zff) + x * y * r.zxy) + c.compton0 * x * (T - c.t_cmb);
+        const float heat = y * N * s.heat_rate;
+        float ed = fabsf(heat - lamK);
+        if (ed * t_left > c.eps_sub * theta) {
+            if (BAIL && ed < c.stiff_kappa * (heat + fabsf(lamK))) return -1;
+            dts = c.eps_sub * theta / ed;
+        }
+    }
+    // backward-Euler coupled (N, x) update, solved for delta = x' - x
+    const float A = s.cs_nH * dts;
+    const float b = dts * r.beta * ne;
+    const float rr = dts * r.alpha * CR * ne;
+    const float L = 1.0f + b + rr;
+    float P = N * s.inv_nH;
+    if (CASE_A) P = fmaf(dts * r.d_alpha * CR * ne, x, P);       // + dts*S_rec/nH
+    const float R0 = rr * x - b * y;
+    const float onepAy = fmaf(A, y, 1.0f);
+    const float a2 = L * A;
+    const float a1 = fmaf(L, onepAy, A * (P - R0));
+    const float a0 = fmaf(P * A, y, -R0 * onepAy);
+    const float disc = f_sqrt(fmaxf(fmaf(a1, a1, -4.0f * a2 * a0), 0.0f));
+    float delta;
+    if (a1 >= 0.0f) delta = 2.0f * a0 * f_rcp(a1 + disc);
+    else delta = (a1 - disc) * f_rcp(2.0f * a2);
+    const float xn = fminf(fmaxf(x + delta, 0.0f), 1.0f);
+    const float yn = fmaxf(y - delta, 0.0f);
+    const float att = f_rcp(fmaf(A, yn, 1.0f));
+    if (BAIL) {
+        // How much the result moves per unit relative error of the sub-step lengths (the fp32 heating estimate that
+        // sets them carries a few 1e-6).  Backward-Euler decay is partition sensitive wherever
+        // rate x dts >> 1:  N' = prod_k (N + s_k)/(1 + A_k y'_k)  moves by  e g_N,  g_N = |s_k/(N + s_k) - A y'/(1 + A y')|
+        // (s_k: the recombination photons of the sub-step), and a recombining x by  e g_x,  g_x = 1 - 1/L.  The LAST
+        // sub-step takes what is left: it inherits minus the summed errors of the others, blown up by
+        // dt/dts_last - 1 when it is a sliver.
+        const float src = CASE_A ? 1.0f - N * s.inv_nH * f_rcp(P) : 0.0f;
+        const float g = fmaxf(fabsf(src - (1.0f - att)), 1.0f - f_rcp(L));
+        if (dts < t_left) {
+            s.sens += g;
+            if (s.sens > c.stiff_sens) return -1;
+        } else if (s.nsub > 0 && s.sens + g * (c.dt * f_rcp(dts) - 1.0f) > c.stiff_sens) {
+            return -1;
+        }
+    }
+    const float Pa = P * att;
+    s.N = nH * Pa;
+    s.att_tot *= att;
+    if (COOL) {
+        const float dth_heat = A * yn * Pa * c.heat_K;
+        const float lamK = nH * (xn * xn * fmaf(CR, r.zrec, r.zff) + xn * yn * r.zxy)
+                           + c.compton0 * xn * (T - c.t_cmb);
+        const float lamK_T = nH * (xn * xn * fmaf(CR, r.zrec_t, r.zff_t) + xn * yn * r.zxy_t)
+                             + c.compton0 * xn * T;
+        // theta' = theta + (dth_heat - dts lamK)/(1 + dts max(0,lamK_T)/theta)
+        const float num = dth_heat - dts * lamK;
+        const float thn = fmaf(num * theta, f_rcp(fmaf(dts, fmaxf(lamK_T, 0.0f), theta)), theta);
+        s.T = fmaxf(thn * f_rcp(1.0f + xn), 1.0f);
+    }
+    s.x = xn;
+    s.y = yn;
+    s.t_left = t_left - dts;
+    ++s.nsub;
+    return (s.t_left > 0.0f && s.nsub < c.max_sub) ? 0 : 1;
+}
+
 template <int FLAGS, bool BAIL = false>
 __device__ __forceinline__ int chemistry(float &N, float &gx, float &gy, float &gz, float &x, float &T,
                                          float nH, const StepConst &c) {
-    constexpr bool CASE_A = FLAGS & F_CASE_A, COOL = FLAGS & F_COOL;
-    const float CR = clumping(nH, c);
-    const float inv_nH = f_rcp(nH);
-    const bool ci_on = c.ci_k0 > 0.0f;
-    const float CI = ci_on ? clumping_i(nH, c) : 1.0f;
-    const float cs_nH = ci_on ? c.cs * nH * CI : c.cs * nH;
-    const float heat_rate = ci_on ? c.heat_rate_K * CI : c.heat_rate_K;
-    float t_left = c.dt;
-    int nsub = 0;
-    float att_tot = 1.0f;
-    float y = 1.0f - x;          // carried: y' = y - delta keeps the neutral fraction's own digits (never 1 - x', H1)
-    float sens = 0.0f;
-    while (t_left > 0.0f && nsub < c.max_sub) {
-        if (BAIL && nsub >= c.stiff_nsub) return -1;
-        Rates r;
-        rates<FLAGS>(T, c, r);
-        const float ne = x * nH;
-        const float theta = (1.0f + x) * T;
-        float dts = t_left;
-        if (COOL) {
-            // estimated net heating rate / (1.5 kB nH)  [K/s]
-            float lamK = nH * (x * x * fmaf(CR, r.zrec, r.zff) + x * y * r.zxy) + c.compton0 * x * (T - c.t_cmb);
-            const float heat = y * N * heat_rate;
-            float ed = fabsf(heat - lamK);
-            if (ed * t_left > c.eps_sub * theta) {
-                if (BAIL && ed < c.stiff_kappa * (heat + fabsf(lamK))) return -1;
-                dts = c.eps_sub * theta / ed;
-            }
-        }
-        // backward-Euler coupled (N, x) update, solved for delta = x' - x
-        const float A = cs_nH * dts;
-        const float b = dts * r.beta * ne;
-        const float rr = dts * r.alpha * CR * ne;
-        const float L = 1.0f + b + rr;
-        float P = N * inv_nH;
-        if (CASE_A) P = fmaf(dts * r.d_alpha * CR * ne, x, P);       // + dts*S_rec/nH
-        const float R0 = rr * x - b * y;
-        const float onepAy = fmaf(A, y, 1.0f);
-        const float a2 = L * A;
-        const float a1 = fmaf(L, onepAy, A * (P - R0));
-        const float a0 = fmaf(P * A, y, -R0 * onepAy);
-        const float disc = f_sqrt(fmaxf(fmaf(a1, a1, -4.0f * a2 * a0), 0.0f));
-        float delta;
-        if (a1 >= 0.0f) delta = 2.0f * a0 * f_rcp(a1 + disc);
-        else delta = (a1 - disc) * f_rcp(2.0f * a2);
-        const float xn = fminf(fmaxf(x + delta, 0.0f), 1.0f);
-        const float yn = fmaxf(y - delta, 0.0f);
-        const float att = f_rcp(fmaf(A, yn, 1.0f));
-        if (BAIL) {
-            // N' = N prod_k 1/(1 + A_k y'_k): a relative error e_k of the k-th sub-step length moves ln N' by
-            // e_k A y'/(1 + A y'), and the fp32 heating estimate carries e_k ~ 4e-6
-            sens += 1.0f - att;
-            if (sens > c.stiff_sens && dts < t_left) return -1;
-        }
-        const float Pa = P * att;
-        N = nH * Pa;
-        att_tot *= att;
-        if (COOL) {
-            const float dth_heat = A * yn * Pa * c.heat_K;
-            const float lamK = nH * (xn * xn * fmaf(CR, r.zrec, r.zff) + xn * yn * r.zxy)
-                               + c.compton0 * xn * (T - c.t_cmb);
-            const float lamK_T = nH * (xn * xn * fmaf(CR, r.zrec_t, r.zff_t) + xn * yn * r.zxy_t)
-                                 + c.compton0 * xn * T;
-            // theta' = theta + (dth_heat - dts lamK)/(1 + dts max(0,lamK_T)/theta)
-            const float num = dth_heat - dts * lamK;
-            const float thn = fmaf(num * theta, f_rcp(fmaf(dts, fmaxf(lamK_T, 0.0f), theta)), theta);
-            T = fmaxf(thn * f_rcp(1.0f + xn), 1.0f);
-        }
-        x = xn;
-        y = yn;
-        t_left -= dts;
-        ++nsub;
-    }
-    gx *= att_tot; gy *= att_tot; gz *= att_tot;
-    return nsub;
+    ChemCell s;
+    chem_begin(s, N, x, T, nH, c);
+    int st;
+    do st = chem_substep<FLAGS, BAIL>(s, c); while (st == 0);
+    if (st < 0) return -1;
+    N = s.N; x = s.x; T = s.T;
+    gx *= s.att_tot; gy *= s.att_tot; gz *= s.att_tot;
+    return s.nsub;
 }
 
 }  // namespace aton

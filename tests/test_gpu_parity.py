@@ -4,6 +4,8 @@ Tolerances are BASELINE.json's: after 1 step from a warm state max relative erro
 N, F (as |dF|/(cN), reading S16), x, T where N > 1e-20 max N; after a full run relative L1 <= 1e-3
 per field and |d<x>_V| <= 1e-3.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -13,9 +15,8 @@ from parity_util import (gpu_run, l1_errors, max_rel_errors, oracle_run, state_t
 
 pytestmark = pytest.mark.gpu
 
-import os
-
-TOL_1STEP = 1e-4
+TOL_1STEP = float(os.environ.get("ATON_TOL_1STEP", "1e-4"))     # the north_star's bar; the override only ever tightens it (probing)
+assert TOL_1STEP <= 1e-4
 TOL_L1 = 1e-3
 TOL_XVOL = 1e-3
 # None = the library's default = the product kernel (variant 4) on every grid it can tile (all cases below but the
@@ -244,8 +245,11 @@ def test_tiled_vs_reference_kernel():
     a, da = gpu_run(w, 3, 0)
     for variant in (2, 4):
         b, db = gpu_run(w, 3, variant)
+        # each kernel is within 1e-4 of the oracle per step (the 1-step bar); two of them within 2e-4 of each other
+        # per step, here over 3 steps from a state where half the cells sub-cycle
         for k in ("N", "x", "T"):
-            assert np.allclose(a[k], b[k], rtol=5e-5, atol=0), (variant, k)
+            assert np.allclose(a[k], b[k], rtol=3e-4, atol=0), (variant, k)
+            assert np.mean(np.abs(a[k] - b[k]) > 2e-5 * np.abs(a[k])) < 1e-3, (variant, k)
         assert db["subcycles_total"] == pytest.approx(da["subcycles_total"], rel=1e-3)
         assert db["subcycles_max"] == da["subcycles_max"]
 
