@@ -6,6 +6,7 @@
 #include "aton_reduce.cuh"
 #include "aton_step_fused.cuh"
 #include "aton_step_v4.cuh"
+#include "aton_step_v5.cuh"
 
 using namespace aton;
 
@@ -89,6 +90,16 @@ StepConstD make_step_const_d(const aton_ctx *ctx, double dt) {
     return s;
 }
 
+// which fused kernel a step launches: 5 (row-wide warps; nx % 128 == 0, ny % 8 == 0), else 4 (32 x 4 / 64 x 2 warp
+// tiles), else 2 (the fallback that tiles anything); variant 0 is the one-thread-per-cell kernel
+int step_kernel_of(const aton_ctx *ctx) {
+    if (ctx->variant == 0) return 0;
+    if (ctx->variant == 5 && v5_pick_w(ctx->g, ctx->tile_y)) return 5;
+    if (ctx->variant == 5 && v4_pick_wxq(ctx->g, 0)) return 4;
+    if (ctx->variant == 4 && v4_pick_wxq(ctx->g, ctx->tile_y)) return 4;
+    return 2;
+}
+
 FieldsIO make_io(const aton_ctx *ctx, int cur) {
     FieldsIO f{};
     const int a = cur, b = 1 - cur;
@@ -101,7 +112,7 @@ FieldsIO make_io(const aton_ctx *ctx, int cur) {
     f.defer_mask = ctx->defer_mask;
     f.src_bits = ctx->src_bits;
     f.stiff_q = ctx->stiff_q; f.stiff_n = ctx->stiff_n; f.stiff_cap = ctx->stiff_cap;
-    f.fix_inject = (ctx->variant == 4 && v4_pick_wxq(ctx->g, ctx->tile_y) != 0) ? 1 : 0;
+    f.fix_inject = step_kernel_of(ctx) >= 4 ? 1 : 0;
     return f;
 }
 
@@ -152,16 +163,19 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
         time_mark(ctx);
         return cudaGetLastError();
     }
-    // variant 4 needs nx % 32 == 0 and ny % 4 == 0 (or nx % 64 == 0 and ny % 2 == 0); other grids run the variant-2
-    // kernel.  Both flag the cells that sub-cycle for step_fixup_kernel; variant 4 also flags its source cells (the
-    // fix-up injects), variant 2 injects in the step kernel.
-    const int wxq4 = ctx->variant == 4 ? v4_pick_wxq(ctx->g, ctx->tile_y) : 0;
+    // variant 5 needs nx % 128 == 0 and ny % 8 == 0, variant 4 nx % 32 == 0 and ny % 4 == 0 (or nx % 64 == 0 and
+    // ny % 2 == 0); other grids run the variant-2 kernel.  All flag the cells that sub-cycle for step_fixup_kernel;
+    // variants 4 and 5 also flag their source cells (the fix-up injects), variant 2 injects in the step kernel.
+    const int kern = step_kernel_of(ctx);
+    const int wxq4 = kern == 4 ? v4_pick_wxq(ctx->g, ctx->variant == 4 ? ctx->tile_y : 0) : (kern == 5 ? -1 : 0);
     if (ctx->slab && !wxq4) return cudaErrorNotSupported;    // checked with a message in aton_step
     ctx->fast_subcycles += (long long)ctx->plane * (ze - zb);
     cudaError_t e;
     time_mark(ctx);
-    if (wxq4)
-        e = launch_step_v4<FLAGS>(f, ctx->g, sc, wxq4, ctx->tile_z, ctx->stream, zb, ze);
+    if (kern == 5)
+        e = launch_step_v5<FLAGS>(f, ctx->g, sc, v5_pick_w(ctx->g, ctx->tile_y), ctx->tile_z, ctx->stream, zb, ze);
+    else if (kern == 4)
+        e = launch_step_v4<FLAGS>(f, ctx->g, sc, wxq4, ctx->variant == 4 ? ctx->tile_z : 0, ctx->stream, zb, ze);
     else
         e = launch_step_fused<FLAGS>(f, ctx->g, sc, ctx->variant == 2 ? ctx->tile_y : 0, ctx->variant == 2 ? ctx->tile_z : 0,
                                      ctx->stream);
@@ -404,9 +418,10 @@ long long aton_launch_count(const aton_t *ctx) { return ctx ? ctx->launches : 0;
 
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z) {
     if (!ctx) return ATON_EINVAL;
-    if (variant != 0 && variant != 2 && variant != 4)
-        return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0, 2 or 4");
-    if ((variant == 2 && !fused_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)))
+    if (variant != 0 && variant != 2 && variant != 4 && variant != 5)
+        return fail(ctx, ATON_EINVAL, "aton_set_kernel: variant must be 0, 2, 4 or 5");
+    if ((variant == 2 && !fused_shape_ok(tile_y, tile_z)) || (variant == 4 && !v4_shape_ok(tile_y, tile_z)) ||
+        (variant == 5 && !v5_shape_ok(tile_y, tile_z)))
         return fail(ctx, ATON_EINVAL, "aton_set_kernel: unsupported tile shape %d x %d", tile_y, tile_z);
     ctx->variant = variant; ctx->tile_y = tile_y; ctx->tile_z = tile_z;
     ctx->fix_dirty = true;
@@ -584,8 +599,8 @@ int aton_step(aton_t *ctx, double dt, int n_steps) {
     if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_step: call aton_set_fields first");
     if (n_steps < 0) return fail(ctx, ATON_EINVAL, "aton_step: n_steps < 0");
     if (int rc = check_dt(ctx, &dt, "aton_step")) return rc;
-    if (ctx->slab && ctx->variant != 4)
-        return fail(ctx, ATON_ESTATE, "aton_step: a slab context runs kernel variant 4 only");
+    if (ctx->slab && ctx->variant != 4 && ctx->variant != 5)
+        return fail(ctx, ATON_ESTATE, "aton_step: a slab context runs kernel variants 4 and 5 only");
     if (ctx->slab && n_steps > 1)
         return fail(ctx, ATON_EINVAL, "aton_step: a slab context advances one step per call (exchange the halo planes first, or use aton_step_slab)");
     if (n_steps > 0) CU(ctx, prepare_step(ctx, dt));

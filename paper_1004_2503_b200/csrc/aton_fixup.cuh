@@ -138,19 +138,23 @@ __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixA
         if (!__syncthreads_or(any != 0u)) continue;       // (the barrier at the loop top orders s_grp's next write)
 #pragma unroll
         for (int k = 0; k < FIXUP_GROUP; k++) {
+            bool full = false;
             if (bits[k]) {
                 const int w = word0 + (grp * FIXUP_GROUP + k) * FIXUP_THREADS + threadIdx.x;
                 f.defer_mask[w] = 0u;
                 unsigned bb = bits[k];
                 int pos = atomicAdd(&qn, __popc(bb));
+                full = pos + __popc(bb) >= FIXUP_QTHRESH;
                 while (bb) {
                     const int b = __ffs(bb) - 1;
                     bb &= bb - 1;
                     queue[pos++] = w * 32 + b;
                 }
             }
-            __syncthreads();
-            if (qn >= FIXUP_QTHRESH) drain();         // uniform: every thread reads the same qn after the barrier
+            // the queue's final length is the largest pos + popc any thread saw: the vote decides for the whole block.
+            // (Reading qn after a plain barrier would race with the next chunk's atomicAdd of a faster thread: part of
+            // the block would drain and the rest would not.)
+            if (__syncthreads_or(full)) drain();
         }
     }
     __syncthreads();

@@ -178,7 +178,8 @@ int aton_step_slab(aton_t *ctx, double dt, int n_steps) {
     if (!ctx->slab || !ctx->comm) return fail(ctx, ATON_ESTATE, "aton_step_slab: needs a slab context with aton_comm_init done");
     if (!ctx->have_fields) return fail(ctx, ATON_ESTATE, "aton_step_slab: call aton_set_fields first");
     if (n_steps < 0) return fail(ctx, ATON_EINVAL, "aton_step_slab: n_steps < 0");
-    if (ctx->variant != 4) return fail(ctx, ATON_ESTATE, "aton_step_slab: a slab context runs kernel variant 4 only");
+    if (ctx->variant != 4 && ctx->variant != 5)
+        return fail(ctx, ATON_ESTATE, "aton_step_slab: a slab context runs kernel variants 4 and 5 only");
     if (int rc = check_dt(ctx, &dt, "aton_step_slab")) return rc;
     cudaSetDevice(ctx->device);
     SlabComm *c = ctx->comm;
