@@ -235,7 +235,7 @@ def run_ours(args, rank, world, local_rank):
     build.build()
     cfg = args.config
     n = args.n or {1: 32, 2: 128, 3: 256, 4: 512, 5: 1024}[cfg]
-    variant = 4 if args.variant is None else args.variant
+    variant = 5 if args.variant is None else args.variant     # 5 = the library default
     slab_mode = args.decomp == "slab"
     if slab_mode:
         # ONE box cut into z slabs, one per rank, halo planes exchanged every step inside the library (aton_step_slab:
@@ -314,7 +314,13 @@ def run_ours(args, rank, world, local_rank):
         return
 
     peak, peak_src = measured_hbm_peak()
-    kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel"}[variant]
+    # the kernel the library launches for this grid (aton_api.cu step_kernel_of): 5 -> 4 -> 2 as the grid allows
+    kvar = variant
+    if kvar == 5 and not (n % 128 == 0):
+        kvar = 4
+    if kvar == 4 and not (n % 32 == 0):
+        kvar = 2
+    kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel", 5: "step_v5_kernel"}[kvar]
     roofline = roofline_of(leg, cells, args.steps, peak, peak_src, recorded_traffic(n, "dark"), kname)
     extra = {}
     if warm:

@@ -122,14 +122,19 @@ int aton_get_fields(aton_t *ctx, float *nH, float *x, float *T, float *N, float 
 /* Global diagnostics of the current state (deterministic two-pass reduction).  Synchronises. */
 int aton_reduce(aton_t *ctx, aton_diag_t *out);
 
-/* Select the step kernel: 4 (default, the product) = warp-autonomous tiles, no inter-warp synchronisation; source
- * cells and cells that need sub-cycling are redone by the producing warp in batches of 32, stiff cells in fp64
- * (needs nx % 32 == 0 and ny % 4 == 0, or nx % 64 == 0 and ny % 2 == 0; any other grid runs the variant-2 kernel);
- * 2 = CTA-tiled fused kernel + mask-scanning fix-up kernel (the fallback for grids variant 4 cannot tile);
+/* Select the step kernel: 5 (default, the product) = row-wide warps (a warp owns a 128-cell row segment, a CTA 8 or 16
+ * rows that exchange their y terms through shared memory behind one mbarrier phase per plane; needs nx % 128 == 0 and
+ * ny % 8 == 0; any other grid falls through to variant 4, then 2);
+ * 4 = warp-autonomous 32 x 4 (or 64 x 2) tiles, no inter-warp synchronisation (needs nx % 32 == 0 and ny % 4 == 0, or
+ * nx % 64 == 0 and ny % 2 == 0; any other grid runs the variant-2 kernel).  Variants 4 and 5 flag their source cells and
+ * the cells that need sub-cycling for step_fixup_kernel (stiff cells go on to the fp64 step_stiff_kernel) and give
+ * bit-identical results;
+ * 2 = CTA-tiled fused kernel + the same fix-up kernels (the fallback for grids the others cannot tile);
  * 0 = reference kernel (one thread per cell, neighbours from global memory; a cross-check).
  * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 14} rows; variant 4: tile_y 4 = 32 x 4
- * warp tiles (default), 2 = 64 x 2; tile_z = planes per z-chunk); results agree between variants to rounding and do
- * not depend on the tile shape (bitwise).  ATON_EINVAL for anything else (variants 1 and 3 of round 1 are gone). */
+ * warp tiles (default), 2 = 64 x 2; variant 5: tile_y 8 (default) or 16 rows per CTA; tile_z = planes per z-chunk);
+ * results agree between variants to rounding and do not depend on the tile shape (bitwise).  ATON_EINVAL for anything
+ * else (variants 1 and 3 of round 1 are gone). */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);
 
 /* Number of kernels launched by the library on this context since aton_init. */

@@ -55,7 +55,7 @@ struct aton_ctx {
     bool have_fields = false;
     long long steps_done = 0, launches = 0;
     double time_s = 0;
-    int variant = 4, tile_y = 0, tile_z = 0;
+    int variant = 5, tile_y = 0, tile_z = 0;
     bool timing = false;                   // aton_set_timing: CUDA events around the kernels of a step
     std::vector<cudaEvent_t> ev;           // pairs (start, stop), one pair per timed launch of the dominant step kernel
     std::vector<cudaEvent_t> ev_fix;       // the same for step_fixup_kernel ...

@@ -53,25 +53,7 @@ __device__ __forceinline__ void rates2(f2 T, bool warm, const StepConst &c, Rate
     const f2 zero = splat(0.0f);
     r.beta = zero;
     r.zrec = r.zff = r.zxy = r.zrec_t = r.zff_t = r.zxy_t = zero;
-    // exp(-157807/T) and exp(-118348/T) underflow fp32 below 1100 K: `warm` (any cell of the thread
-    // above 1100 K) only skips work, the skipped terms are exact zeros.
-    f2 invT = zero, lam = zero;
-    if ((COLL || COOL) && warm) {
-        invT = rcp2(T);
-        lam = invT * 315614.0f;
-    }
-    f2 zci = zero, zci_t = zero;
-    if (COLL && warm) {
-        const f2 u = ex22(fma2(l2lam, 0.874f, 0.874f * 1.49817873f));      // (lam/0.354)^0.874
-        const f2 lu = lg22(u + 1.0f);
-        // log2 of T^-1.5 exp(-lam/2) lam^-1.089 / (1+u)^1.101
-        const f2 e = fma2(l2T, -1.5f, fma2(lam, -0.72134752f, fma2(l2lam, -1.089f, lu * -1.101f)));
-        r.beta = ex22(e + 4.39985467f);                                    // * 21.11
-        if (COOL) {
-            zci = r.beta * c.zci_over_beta;                                // 13.6 eV / (1.5 kB)
-            zci_t = zci * (fma2(lam, 0.5f, -0.411f) + (u * 0.962274f) * rcp2(u + 1.0f));
-        }
-    }
+    f2 sqT = zero;
     if (COOL) {
         // recombination cooling K T lam^p / (1+u)^r ; d ln/d ln T = 1 - p + r q u/(1+u)
         constexpr float q = CASE_A ? 0.502f : 0.376f, l0 = CASE_A ? 0.88629950f : -1.16992500f;
@@ -81,22 +63,38 @@ __device__ __forceinline__ void rates2(f2 T, bool warm, const StepConst &c, Rate
         r.zrec = ex22((l2T + c.l2_zrec0) + fma2(l2lam, p, lu * -rr));
         r.zrec_t = r.zrec * fma2(u * (rr * q), rcp2(u + 1.0f), 1.0f - p);
         // bremsstrahlung with Gaunt factor: zff0 gff sqrt(T); zff_t = zff/2 + zff0 sqrt(T) gau d (2/3)/ln10
-        const f2 sqT = sqrt2(T);
+        sqT = sqrt2(T);
         const f2 d = fma2(l2T, -0.30102999f, 5.5f);                         // 5.5 - log10 T
         const f2 gau = ex22((d * d) * -0.48089835f) * 0.34f;               // 0.34 exp(-d^2/3)
         const f2 zs = sqT * c.zff0;
         r.zff = zs * (gau + 1.1f);
         r.zff_t = fma2(r.zff, 0.5f, (zs * gau) * (d * 0.28952965f));
-        // collisional excitation
-        f2 zex = zero, zex_t = zero;
-        if (warm) {
-            const f2 pw = sqT * 3.16227766e-3f;                             // sqrt(T/1e5)
-            const f2 ipw = rcp2(pw + 1.0f);
-            zex = (ex22(invT * -170740.07f) * c.zexc0) * ipw;              // 118348 * log2(e)
-            zex_t = zex * fma2(invT, 118348.0f, (pw * ipw) * -0.5f);
+    }
+    // exp(-157807/T) and exp(-118348/T) underflow fp32 below 1100 K: `warm` (any cell of the thread above 1100 K) only
+    // skips work, the skipped terms are exact zeros.  One branch holds all of it.
+    if ((COLL || COOL) && warm) {
+        const f2 invT = rcp2(T);
+        f2 zci = zero, zci_t = zero;
+        if (COLL) {
+            const f2 lam = invT * 315614.0f;
+            const f2 u = ex22(fma2(l2lam, 0.874f, 0.874f * 1.49817873f));      // (lam/0.354)^0.874
+            const f2 lu = lg22(u + 1.0f);
+            // log2 of T^-1.5 exp(-lam/2) lam^-1.089 / (1+u)^1.101
+            const f2 e = fma2(l2T, -1.5f, fma2(lam, -0.72134752f, fma2(l2lam, -1.089f, lu * -1.101f)));
+            r.beta = ex22(e + 4.39985467f);                                    // * 21.11
+            if (COOL) {
+                zci = r.beta * c.zci_over_beta;                                // 13.6 eV / (1.5 kB)
+                zci_t = zci * (fma2(lam, 0.5f, -0.411f) + (u * 0.962274f) * rcp2(u + 1.0f));
+            }
         }
-        r.zxy = zex + zci;
-        r.zxy_t = zex_t + zci_t;
+        if (COOL) {     // collisional excitation
+            const f2 pw = sqT * 3.16227766e-3f;                                 // sqrt(T/1e5)
+            const f2 ipw = rcp2(pw + 1.0f);
+            const f2 zex = (ex22(invT * -170740.07f) * c.zexc0) * ipw;         // 118348 * log2(e)
+            const f2 zex_t = zex * fma2(invT, 118348.0f, (pw * ipw) * -0.5f);
+            r.zxy = zex + zci;
+            r.zxy_t = zex_t + zci_t;
+        }
     }
 }
 
@@ -175,7 +173,9 @@ __device__ __forceinline__ unsigned chem_fast2(f2 &N, f2 &gx, f2 &gy, f2 &gz, f2
         Tn = max2(thn * rcp2(xn + 1.0f), 1.0f);
     }
     const f2 Nn = nH * Pa, gxn = gx * att, gyn = gy * att, gzn = gz * att;
-    {   // branch-free: a deferred half keeps its input values
+    if (defer == 0u) {      // the common case by far: nothing to keep, no selects
+        N = Nn; gx = gxn; gy = gyn; gz = gzn; x = xn; T = Tn;
+    } else {                // a deferred half keeps its input values
         const bool k0 = defer & 1u, k1 = defer & 2u;
 #define ATON_KEEP(old, nw) old = pk(k0 ? lo(old) : lo(nw), k1 ? hi(old) : hi(nw))
         ATON_KEEP(N, Nn); ATON_KEEP(gx, gxn); ATON_KEEP(gy, gyn); ATON_KEEP(gz, gzn);

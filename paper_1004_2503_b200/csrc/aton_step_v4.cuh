@@ -89,6 +89,18 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
     asm volatile("{\n.reg .pred p;\nsetp.ne.s32 p, %2, 0;\n@p cp.async.ca.shared.global [%0], [%1], 4;\n}"
                  ::"r"(smem_u32(smem)), "l"(gmem), "r"(pred) : "memory");
 }
+// x, T, n_H, source bits of the plane being finished staged by cp.async through the slots of the plane just read: no
+// register is held while they travel.  Pays in variant 5 (12.98 -> 12.4 ms per 1024^3 launch), not here (13.2 -> 13.45 ms:
+// the extra LDGSTS compete with the halo re-reads for this kernel's L1): profiles/r02_d_latency.md
+#ifndef ATON_V4_XT
+#define ATON_V4_XT 0
+#endif
+#ifndef ATON_V5_XT
+#define ATON_V5_XT 1
+#endif
+#ifndef ATON_PF
+#define ATON_PF 1        // L2 prefetch of x, T, n_H, source bits two planes ahead: 1 per thread (prefetch.global.L2), 2 bulk per row
+#endif
 #ifndef ATON_V4_MINB
 #define ATON_V4_MINB 4
 #endif
@@ -148,6 +160,21 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
             }
 #endif
         }
+#if ATON_PF == 1
+        if (inpl) {      // the plane is finished two iterations from now: its x, T, n_H and source bits wait in L2 by then
+            prefetch_l2(f.x + base + rowoff);
+            prefetch_l2(f.T + base + rowoff);
+            prefetch_l2(f.nH + base + rowoff);
+            if (q == 0) prefetch_l2(f.src_bits + ((unsigned)(base + rowoff) >> 5));
+        }
+#elif ATON_PF == 2
+        if (inpl && q == 0) {
+            prefetch_l2_bulk(f.x + base + rowoff, 4 * C::WX);
+            prefetch_l2_bulk(f.T + base + rowoff, 4 * C::WX);
+            prefetch_l2_bulk(f.nH + base + rowoff, 4 * C::WX);
+            prefetch_l2(f.src_bits + ((unsigned)(base + rowoff) >> 5));
+        }
+#endif
         cp_async_commit();
         kst = kst + 1 == g.nz ? 0 : kst + 1;
     };
@@ -168,32 +195,41 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     auto iter = [&](auto inpl_tag, auto fin_tag, bool stage_next, bool next_inpl) {
         constexpr bool INPL = decltype(inpl_tag)::value, FIN = decltype(fin_tag)::value;
         cp_async_wait_all();                             // this thread's part of plane m has landed
-        const float *buf = raw + (m & 1) * C::RAW_BUF;
+        float *buf = raw + (m & 1) * C::RAW_BUF;
+        // the staged quad of plane m goes to registers first: its slots are reused right away
+        const float4 n4 = *reinterpret_cast<const float4 *>(buf + my);
+        const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + my);
+        const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + my);
+        const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + my);
+#if ATON_V4_XT
+        // x, T, n_H and the source bits of plane m-1 (finished at the end of this iteration) travel through the slots
+        // just read: no register is held while they are on their way (profiles/r02_d_latency.md).  (The lanes of the
+        // middle rows re-read their own slot in the halo pass below: whatever they find there is never stored.)
+        if (FIN) {
+            cp_async16(buf + my, f.x + oprev);
+            cp_async16(buf + C::RAW_FIELD + my, f.T + oprev);
+            cp_async16(buf + 2 * C::RAW_FIELD + my, f.nH + oprev);
+            cp_async4(buf + 3 * C::RAW_FIELD + my, f.src_bits + ((unsigned)oprev >> 5));
+            cp_async_commit();
+        }
+#endif
         if (stage_next) stage(m + 1, next_inpl);
 
+#if !ATON_V4_XT
         // early loads for the chemistry of plane m-1
         float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), T4 = x4, h4 = make_float4(1.f, 1.f, 1.f, 1.f);
         unsigned srcw = 0;
         if (FIN) {
-#if ATON_V4_CS & 1       // read once: streaming loads keep the (N, G) rows that tile halos re-read in L2
-            x4 = __ldcs(reinterpret_cast<const float4 *>(f.x + oprev));
-            T4 = __ldcs(reinterpret_cast<const float4 *>(f.T + oprev));
-            h4 = __ldcs(reinterpret_cast<const float4 *>(f.nH + oprev));
-#else
             x4 = *reinterpret_cast<const float4 *>(f.x + oprev);
             T4 = *reinterpret_cast<const float4 *>(f.T + oprev);
             h4 = __ldg(reinterpret_cast<const float4 *>(f.nH + oprev));
-#endif
             srcw = __ldg(f.src_bits + ((unsigned)oprev >> 5));
         }
+#endif
         // ---- closure of the staged quad
         Quad u;
         f2 a[2], s[2];
         {
-            const float4 n4 = *reinterpret_cast<const float4 *>(buf + my);
-            const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + my);
-            const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + my);
-            const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + my);
 #pragma unroll
             for (int p = 0; p < 2; p++) {
                 u.v[p][0] = ld_pair(n4, p); u.v[p][1] = ld_pair(gx4, p);
@@ -311,6 +347,13 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         // ---- plane m-1 has all six contributions: one chemistry sub-step, store; source cells and cells
         //      that need sub-cycling keep their transported (N, G), old (x, T) and are flagged
         if (FIN) {
+#if ATON_V4_XT
+            if (stage_next) cp_async_wait_1(); else cp_async_wait_all();     // the next plane's staging may still fly
+            const float4 x4 = *reinterpret_cast<const float4 *>(buf + my);
+            const float4 T4 = *reinterpret_cast<const float4 *>(buf + C::RAW_FIELD + my);
+            const float4 h4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RAW_FIELD + my);
+            const unsigned srcw = *reinterpret_cast<const unsigned *>(buf + 3 * C::RAW_FIELD + my);
+#endif
             const unsigned srcn = (srcw >> (oprev & 31)) & 0xFu;
             f2 xs[2] = {pk(x4.x, x4.y), pk(x4.z, x4.w)}, Ts[2] = {pk(T4.x, T4.y), pk(T4.z, T4.w)};
             const f2 hs[2] = {pk(h4.x, h4.y), pk(h4.z, h4.w)};

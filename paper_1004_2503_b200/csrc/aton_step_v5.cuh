@@ -46,11 +46,23 @@ __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned coun
 __device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
     asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.release.cta.shared::cta.b64 st, [%0];\n}" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+#ifndef ATON_V5_SLEEP_NS
+#define ATON_V5_SLEEP_NS 64u    // back-off of a warp that is ahead of its CTA: it sleeps instead of spinning through issue slots
+#endif
+__device__ __forceinline__ bool mbar_test(unsigned long long *bar, unsigned parity) {
+    unsigned ok;
     asm volatile(
-        "{\n.reg .pred p;\nWAIT_%=:\n"
-        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%0], %1;\n"
-        "@!p bra WAIT_%=;\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+        "{\n.reg .pred p;\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    while (!mbar_test(bar, parity)) {
+#if ATON_V5_SLEEP_NS > 0
+        __nanosleep(ATON_V5_SLEEP_NS);
+#endif
+    }
 }
 
 template <int FLAGS, int W>
@@ -102,6 +114,21 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
                 for (int v = 0; v < 4; v++) cp_async16(hd + v * C::WX, src[v] + ho);
             }
         }
+#if ATON_PF == 1
+        if (inpl) {      // the plane is finished two iterations from now: its x, T, n_H and source bits wait in L2 by then
+            prefetch_l2(f.x + base + rowoff);
+            prefetch_l2(f.T + base + rowoff);
+            prefetch_l2(f.nH + base + rowoff);
+            if ((q & 7) == 0) prefetch_l2(f.src_bits + ((unsigned)(base + rowoff) >> 5));
+        }
+#elif ATON_PF == 2
+        if (inpl && q == 0) {
+            prefetch_l2_bulk(f.x + base + rowoff, 4 * C::WX);
+            prefetch_l2_bulk(f.T + base + rowoff, 4 * C::WX);
+            prefetch_l2_bulk(f.nH + base + rowoff, 4 * C::WX);
+            prefetch_l2_bulk(f.src_bits + ((unsigned)(base + rowoff) >> 5), 16);
+        }
+#endif
         cp_async_commit();
         kst = kst + 1 == g.nz ? 0 : kst + 1;
     };
@@ -125,9 +152,26 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         // every row has published plane m-1 (and with that has consumed plane m-2: the patch of parity m & 1 and the
         // halo staging of parity (m + 1) & 1 are free)
         if (FIN) mbar_wait(bar, (unsigned)(m & 1));
-        const float *buf = raw + (m & 1) * C::RAW_BUF;
+        float *buf = raw + (m & 1) * C::RAW_BUF;
+        // the staged quad of plane m goes to registers first: its slots are reused right away
+        const float4 n4 = *reinterpret_cast<const float4 *>(buf + my);
+        const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RS + my);
+        const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RS + my);
+        const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RS + my);
+#if ATON_V5_XT
+        // x, T, n_H and the source bits of plane m-1 (finished at the end of this iteration) travel through the slots
+        // just read: no register is held while they are on their way (profiles/r02_d_latency.md)
+        if (FIN) {
+            cp_async16(buf + my, f.x + oprev);
+            cp_async16(buf + C::RS + my, f.T + oprev);
+            cp_async16(buf + 2 * C::RS + my, f.nH + oprev);
+            cp_async4(buf + 3 * C::RS + my, f.src_bits + ((unsigned)oprev >> 5));
+            cp_async_commit();
+        }
+#endif
         if (stage_next) stage(m + 1, next_inpl);
 
+#if !ATON_V5_XT
         // early loads for the chemistry of plane m-1
         float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f), T4 = x4, h4 = make_float4(1.f, 1.f, 1.f, 1.f);
         unsigned srcw = 0;
@@ -137,6 +181,7 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
             h4 = __ldg(reinterpret_cast<const float4 *>(f.nH + oprev));
             srcw = __ldg(f.src_bits + ((unsigned)oprev >> 5));
         }
+#endif
         // ---- y terms of plane m-1 from the rows below and above (published one iteration ago)
         if (FIN) {
             const float *yp = ypat + ((m - 1) & 1) * C::Y_PAR + warp * C::WX + 4 * q, *ym = yp + C::Y_SIGN;
@@ -153,10 +198,6 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         Quad u;
         f2 a[2], s[2];
         {
-            const float4 n4 = *reinterpret_cast<const float4 *>(buf + my);
-            const float4 gx4 = *reinterpret_cast<const float4 *>(buf + C::RS + my);
-            const float4 gy4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RS + my);
-            const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RS + my);
 #pragma unroll
             for (int p = 0; p < 2; p++) {
                 u.v[p][0] = ld_pair(n4, p); u.v[p][1] = ld_pair(gx4, p);
@@ -255,6 +296,13 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         // ---- plane m-1 has all six contributions: one chemistry sub-step, store; source cells and cells
         //      that need sub-cycling keep their transported (N, G), old (x, T) and are flagged
         if (FIN) {
+#if ATON_V5_XT
+            if (stage_next) cp_async_wait_1(); else cp_async_wait_all();     // the next plane's staging may still fly
+            const float4 x4 = *reinterpret_cast<const float4 *>(buf + my);
+            const float4 T4 = *reinterpret_cast<const float4 *>(buf + C::RS + my);
+            const float4 h4 = *reinterpret_cast<const float4 *>(buf + 2 * C::RS + my);
+            const unsigned srcw = *reinterpret_cast<const unsigned *>(buf + 3 * C::RS + my);
+#endif
             const unsigned srcn = (srcw >> (oprev & 31)) & 0xFu;
             f2 xs[2] = {pk(x4.x, x4.y), pk(x4.z, x4.w)}, Ts[2] = {pk(T4.x, T4.y), pk(T4.z, T4.w)};
             const f2 hs[2] = {pk(h4.x, h4.y), pk(h4.z, h4.w)};
