@@ -78,7 +78,7 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
         for line in self.f:
             c = [t.strip() for t in line.split(",")]
@@ -88,14 +88,19 @@ class ClockSampler:
                 sm.append(float(c[0])); mx.append(float(c[1]))
             except ValueError:
                 continue
+            try:
+                pw.append(float(c[2]))
+            except ValueError:
+                pass
             for nm, v in zip(names, c[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         self.f.close()
         os.unlink(self.f.name)
         sm.sort()
+        pw.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w": pw[len(pw) // 2] if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def max_over_ranks(value: float, world: int) -> float:

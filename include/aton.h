@@ -132,7 +132,7 @@ int aton_reduce(aton_t *ctx, aton_diag_t *out);
  * 2 = CTA-tiled fused kernel + the same fix-up kernels (the fallback for grids the others cannot tile);
  * 0 = reference kernel (one thread per cell, neighbours from global memory; a cross-check).
  * tile_y / tile_z choose the tile shape (0 = default; variant 2: tile_y in {6, 14} rows; variant 4: tile_y 4 = 32 x 4
- * warp tiles (default), 2 = 64 x 2; variant 5: tile_y 8 (default) or 16 rows per CTA; tile_z = planes per z-chunk);
+ * warp tiles (default), 2 = 64 x 2; variant 5: tile_y 16 (default when ny % 16 == 0) or 8 rows per CTA; tile_z = planes per z-chunk);
  * results agree between variants to rounding and do not depend on the tile shape (bitwise).  ATON_EINVAL for anything
  * else (variants 1 and 3 of round 1 are gone). */
 int aton_set_kernel(aton_t *ctx, int variant, int tile_y, int tile_z);

@@ -13,7 +13,7 @@ __device__ __forceinline__ void cp_async4(void *smem, const void *gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
 }
 // L2 prefetches of data a later iteration reads with plain loads (x, T, n_H, the source bits): no register and no shared
-// memory is held while the line travels from HBM (profiles/r02_d_prefetch.md)
+// memory is held while the line travels from HBM (profiles/r02_d_step_v5.md)
 __device__ __forceinline__ void prefetch_l2(const void *gmem) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(gmem));
 }

@@ -91,7 +91,7 @@ __device__ __forceinline__ void cp_async4_if(void *smem, const void *gmem, int p
 }
 // x, T, n_H, source bits of the plane being finished staged by cp.async through the slots of the plane just read: no
 // register is held while they travel.  Pays in variant 5 (12.98 -> 12.4 ms per 1024^3 launch), not here (13.2 -> 13.45 ms:
-// the extra LDGSTS compete with the halo re-reads for this kernel's L1): profiles/r02_d_latency.md
+// the extra LDGSTS compete with the halo re-reads for this kernel's L1): profiles/r02_d_step_v5.md
 #ifndef ATON_V4_XT
 #define ATON_V4_XT 0
 #endif
@@ -203,7 +203,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RAW_FIELD + my);
 #if ATON_V4_XT
         // x, T, n_H and the source bits of plane m-1 (finished at the end of this iteration) travel through the slots
-        // just read: no register is held while they are on their way (profiles/r02_d_latency.md).  (The lanes of the
+        // just read: no register is held while they are on their way (profiles/r02_d_step_v5.md).  (The lanes of the
         // middle rows re-read their own slot in the halo pass below: whatever they find there is never stored.)
         if (FIN) {
             cp_async16(buf + my, f.x + oprev);

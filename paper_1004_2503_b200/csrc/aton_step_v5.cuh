@@ -1,24 +1,30 @@
-// Fused step kernel, variant 5: ROW-WIDE warps, CTA-shared y terms consumed one plane late.
+// Fused step kernel, variant 5 (the PRODUCT kernel for grids with nx % 128 == 0 and ny % 8 == 0): ROW-WIDE warps,
+// CTA-shared y terms consumed one plane late.  Transport + one chemistry sub-step in one pass over HBM (52 B per cell-update).
 //
-// Why (profiles/r01_e_tile_shape.md, r02_c_step_v4.md): variant 4's warp-autonomous 32 x 4 tile pays twice for its
-// independence.  (i) Every warp request is four 128-byte row segments, and a z-march made of those streams at 0.83 of
+// Why (profiles/r01_e_tile_shape.md, r02_c_step_v4.md, r02_d_step_v5.md): variant 4's warp-autonomous 32 x 4 tile pays twice
+// for its independence.  (i) Every warp request is four 128-byte row segments, and a z-march made of those streams at 0.83 of
 // the copy peak (10.4 ms per 1024^3 step against 8.7 ms for 256- or 512-byte segments).  (ii) Every warp closes its own
 // tile halo: three extra closure + flux passes per plane on top of the two of its own cells (17 % of the kernel's MUFU
 // work).  Here
 //  * a warp owns ONE ROW SEGMENT of 128 cells (lane q = the quad of cells 4q .. 4q+3): every load, cp.async and store of
 //    a warp is 512 contiguous bytes; x neighbours by shuffles across the whole warp, z neighbours in registers;
-//  * a CTA is W warps stacked in y (W = 8: a 128 x 8 tile, two CTAs per SM).  Every row publishes (U + F_y) and
-//    (U - F_y) of plane m to a CTA-shared patch (double buffered by plane parity) and picks up its neighbours' terms
-//    ONE ITERATION LATER, when plane m-1 is completed anyway (its +z term arrives with plane m).  The only inter-warp
-//    synchronisation is one mbarrier phase per plane, arrived on right after the publish and waited for at the top of
-//    the NEXT iteration: a warp may run a whole iteration ahead of its slowest neighbour before it stalls
-//    (variant 3 of round 1 synchronised inside the iteration and lost 20 % of its issue slots to the barrier);
+//  * a CTA is W warps stacked in y (W = 16: a 128 x 16 tile, one CTA per SM; W = 8 when ny % 16 != 0, two per SM).  Every
+//    row publishes (U + F_y) and (U - F_y) of plane m to a CTA-shared patch (double buffered by plane parity) and picks up
+//    its neighbours' terms ONE ITERATION LATER, when plane m-1 is completed anyway (its +z term arrives with plane m).  The
+//    only inter-warp synchronisation is one mbarrier phase per plane, arrived on right after the publish and waited for at
+//    the top of the NEXT iteration: a warp may run a whole iteration ahead of its slowest neighbour before it stalls
+//    (variant 3 of round 1 synchronised inside the iteration and lost 20 % of its issue slots to the barrier); a warp that
+//    has to wait sleeps between probes;
 //  * the two y halo rows of the CTA tile are closed by ONE warp each, a duty that rotates with the plane index
 //    (below: warp m mod W, above: warp (m + W/2) mod W): 2 / W extra passes per warp and plane instead of 2;
-//  * everything else is variant 4's: thread-private cp.async staging one plane ahead, the peeled z loop, the x halo
-//    cell of the edge lanes, one straight-line chemistry sub-step (chem_fast2), source cells and cells that sub-cycle
-//    flagged in the 1-bit mask for step_fixup_kernel.  The additions reach the accumulators in variant 4's order:
-//    results are bit-identical to variant 4's.
+//  * NO PLAIN GLOBAL LOAD in the loop: (N, G) of plane m+1 are staged by cp.async one plane ahead into thread-private
+//    double-buffered slots; as soon as the quad of plane m has been read into registers its four slots receive x, T, n_H and
+//    the source word of plane m-1 (the plane this iteration finishes) by cp.async too, fetched from L2 where a prefetch put
+//    them two planes earlier.  No register waits for memory: with plain loads ptxas sank them to within 17-270 instructions
+//    of their first use and every warp spent 27 % of its time on that scoreboard (profiles/r02_d_step_v5.md);
+//  * everything else is variant 4's: the peeled z loop, the x halo cell of the edge lanes, one straight-line chemistry
+//    sub-step (chem_fast2), source cells and cells that sub-cycle flagged in the 1-bit mask for step_fixup_kernel.  The
+//    additions reach the accumulators in variant 4's order: results are bit-identical to variant 4's.
 #pragma once
 #include "aton_step_v4.cuh"
 
@@ -160,7 +166,7 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
         const float4 gz4 = *reinterpret_cast<const float4 *>(buf + 3 * C::RS + my);
 #if ATON_V5_XT
         // x, T, n_H and the source bits of plane m-1 (finished at the end of this iteration) travel through the slots
-        // just read: no register is held while they are on their way (profiles/r02_d_latency.md)
+        // just read: no register is held while they are on their way (profiles/r02_d_step_v5.md)
         if (FIN) {
             cp_async16(buf + my, f.x + oprev);
             cp_async16(buf + C::RS + my, f.T + oprev);
@@ -338,11 +344,12 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     iter(no, yes, false, false);               // m = lzn + 1: z halo plane above, finishes plane lzn
 }
 
-// grids variant 5 tiles: nx % 128 == 0 and ny % W == 0 (W = 8 rows per CTA; tile_y = 16 asks for W = 16)
+// grids variant 5 tiles: nx % 128 == 0 and ny % W == 0 (W = 16 rows per CTA when ny allows it, else 8; tile_y forces one)
 inline int v5_pick_w(const Grid &g, int tile_y) {
     if (g.nx % 128 != 0) return 0;
     if (tile_y == 16) return g.ny % 16 == 0 ? 16 : 0;
-    if (tile_y == 0 || tile_y == 8) return g.ny % 8 == 0 ? 8 : 0;
+    if (tile_y == 8) return g.ny % 8 == 0 ? 8 : 0;
+    if (tile_y == 0) return g.ny % 16 == 0 ? 16 : (g.ny % 8 == 0 ? 8 : 0);   // 16 rows: 12.17 against 12.35 ms at 1024^3
     return 0;
 }
 inline bool v5_shape_ok(int tile_y, int tile_z) { return (tile_y == 0 || tile_y == 8 || tile_y == 16) && tile_z >= 0; }
@@ -352,7 +359,7 @@ inline int v5_default_lz(const Grid &g, int tile_z, int nzr) {
     if (tile_z > 0) return tile_z < nzr ? tile_z : nzr;
     const long tiles_xy = (long)(g.nx / 128) * (g.ny / W);
     const long per_wave = 148L * (512 / (32 * W));
-    int lz = 64;      // largest power of two <= 64 that still gives >= 4 waves
+    int lz = 128;     // largest power of two <= 128 that still gives >= 4 waves
     while (lz > 4 && tiles_xy * ((nzr + lz - 1) / lz) < 4 * per_wave) lz >>= 1;
     return lz < nzr ? lz : nzr;
 }
