@@ -81,7 +81,9 @@ def _case(nx, ny, nz, seed=2):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("shape,world", [((64, 8, 12), 2), ((32, 12, 13), 3), ((64, 8, 5), 5), ((32, 8, 9), 1)])
+# 128-wide grids run the product kernel (variant 5: 16 or 8 rows per CTA), the others the variant-4 fallback
+@pytest.mark.parametrize("shape,world", [((64, 8, 12), 2), ((32, 12, 13), 3), ((64, 8, 5), 5), ((32, 8, 9), 1),
+                                         ((128, 16, 12), 2), ((128, 8, 10), 3), ((256, 32, 7), 2)])
 def test_slabs_on_one_gpu_equal_the_undivided_run(shape, world):
     from paper_1004_2503_b200 import aton
     nx, ny, nz = shape
@@ -179,13 +181,14 @@ def test_slab_class_world_size_1_and_errors():
 
 
 @pytest.mark.gpu
-def test_native_slab_step_with_nccl_self_exchange_against_the_oracle(orc):
+@pytest.mark.parametrize("shape", [(64, 16, 10), (128, 16, 10)], ids=["v4_64x16x10", "v5_128x16x10"])
+def test_native_slab_step_with_nccl_self_exchange_against_the_oracle(orc, shape):
     """aton_step_slab through a real NCCL communicator (one rank: every send pairs with the rank's own receive, the same
     code path as N ranks) on a grid with several z planes per launch range, against the ORACLE (not only the undivided
     CUDA run): relative L1 <= 1e-3 after 30 steps, and bit-identical to the undivided CUDA run."""
     from paper_1004_2503_b200 import aton
     from parity_util import l1_errors
-    nx, ny, nz = 64, 16, 10
+    nx, ny, nz = shape
     nH, p, dx, pos, rate = _case(nx, ny, nz, seed=9)
     x0, T0 = torch.full_like(nH, 1e-3), torch.full_like(nH, 100.0)
     dt, steps = wl.courant_dt(dx), 30
