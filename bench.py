@@ -54,23 +54,31 @@ def recorded_traffic(n, state):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons (B200_PROFILING.md), sampled every 50 ms from before the warm-up on; stop()
+    keeps the samples whose time stamp falls inside the timed windows given to it (the timed steps and the second pass
+    of the same steps with the per-kernel events; nvidia-smi needs ~0.3 s to start, longer than a short timed region)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.windows = []
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
+    def window(self, t0, t1):
+        self.windows.append((t0, t1))
+
     def stop(self):
+        import datetime
         if self.p is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)          # let the sample that covers the end of the last window arrive
         self.p.terminate()
         try:
             self.p.wait(timeout=5)
@@ -78,29 +86,34 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, pw, reasons = [], [], [], set()
+        rows = []
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
         for line in self.f:
             c = [t.strip() for t in line.split(",")]
-            if len(c) < 7:
+            if len(c) < 8:
                 continue
             try:
-                sm.append(float(c[0])); mx.append(float(c[1]))
+                ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                sm, mx = float(c[1]), float(c[2])
             except ValueError:
                 continue
             try:
-                pw.append(float(c[2]))
+                pw = float(c[3])
             except ValueError:
-                pass
-            for nm, v in zip(names, c[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
+                pw = None
+            rows.append((ts, sm, mx, pw, [nm for nm, v in zip(names, c[4:8]) if v.lower().startswith("active")]))
         self.f.close()
         os.unlink(self.f.name)
-        sm.sort()
-        pw.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w": pw[len(pw) // 2] if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        inside = [r for r in rows if any(t0 <= r[0] <= t1 for t0, t1 in self.windows)]
+        where = "timed steps + per-kernel timing pass of the same steps"
+        if len(inside) < 2:       # a very short run: fall back to every sample taken under load (warm-up included)
+            inside = [r for r in rows if r[3] is not None and r[3] > 400.0] or rows
+            where = "all samples under load (timed region shorter than the sampling period)"
+        sm = sorted(r[1] for r in inside)
+        pw = sorted(r[3] for r in inside if r[3] is not None)
+        reasons = sorted({nm for r in inside for nm in r[4]})
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max((r[2] for r in inside), default=None),
+                "power_w": pw[len(pw) // 2] if pw else None, "samples": len(sm), "window": where, "reasons": reasons}
 
 
 def max_over_ranks(value: float, world: int) -> float:
@@ -183,31 +196,39 @@ def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0):
     """W untimed + K timed steps (device time, barrier + synchronize on both sides), then the same K steps again with
     the library's own events around each kernel.  Returns a dict of this rank's numbers."""
     import torch
+    sampler = ClockSampler(sampler_rank0) if sampler_rank0 is not None else None
     do_step(dt, warmup)
     torch.cuda.synchronize()
     if world > 1:
         torch.distributed.barrier()
-    sampler = ClockSampler(sampler_rank0) if sampler_rank0 is not None else None
     l0 = a.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    w0 = time.time()
     e0.record(stream)
     do_step(dt, steps)
     e1.record(stream)
     torch.cuda.synchronize()
+    w1 = time.time()
     if world > 1:
         torch.distributed.barrier()
     ms_total = e0.elapsed_time(e1)
     launches = a.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
     d0 = a.reduce()
     # the kernels alone: CUDA events on the library's stream around each launch (aton_set_timing), in a second pass
     # of the same K steps so the events stay out of `value`
     a.set_timing(True)
+    w2 = time.time()
     do_step(dt, steps)
     k_ms, k_n = a.kernel_time()
     f_ms, s_ms, f_n = a.fixup_time()
+    w3 = time.time()
     a.set_timing(False)
+    clocks = None
+    if sampler:
+        sampler.window(w0, w1)
+        sampler.window(w2, w3)
+        clocks = sampler.stop()
     d1 = a.reduce()
     per = lambda k: (d1[k] - d0[k]) / max(steps, 1)
     return {"ms_total": ms_total, "launches": launches, "clocks": clocks, "diag": d0,
