@@ -192,9 +192,11 @@ def run_reference(args, rank, world):
 
 
 # ------------------------------------------------------------------------------------------ ours
-def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0):
-    """W untimed + K timed steps (device time, barrier + synchronize on both sides), then the same K steps again with
-    the library's own events around each kernel.  Returns a dict of this rank's numbers."""
+def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0, rewind=None):
+    """W untimed + K timed steps (device time, barrier + synchronize on both sides), then K steps again with the
+    library's own events around each kernel: the next K steps of the run, or -- with `rewind`, a callable that restores
+    the leg's start state -- the very same W + K steps (the warm leg's state relaxes quickly: its fix-up load halves
+    within tens of steps).  Returns a dict of this rank's numbers."""
     import torch
     sampler = ClockSampler(sampler_rank0) if sampler_rank0 is not None else None
     do_step(dt, warmup)
@@ -217,6 +219,11 @@ def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0):
     d0 = a.reduce()
     # the kernels alone: CUDA events on the library's stream around each launch (aton_set_timing), in a second pass
     # of the same K steps so the events stay out of `value`
+    if rewind is not None:
+        rewind()
+        do_step(dt, warmup)
+        torch.cuda.synchronize()
+    dA = a.reduce()           # counters at the start of the second pass
     a.set_timing(True)
     w2 = time.time()
     do_step(dt, steps)
@@ -230,7 +237,7 @@ def timed_leg(a, do_step, dt, steps, warmup, world, stream, sampler_rank0):
         sampler.window(w2, w3)
         clocks = sampler.stop()
     d1 = a.reduce()
-    per = lambda k: (d1[k] - d0[k]) / max(steps, 1)
+    per = lambda k: (d1[k] - dA[k]) / max(steps, 1)
     return {"ms_total": ms_total, "launches": launches, "clocks": clocks, "diag": d0,
             "kernel_ms": k_ms / max(k_n, 1), "kernel_launches": k_n,
             "fixup_ms": f_ms / max(f_n, 1), "stiff_ms": s_ms / max(f_n, 1),
@@ -329,11 +336,14 @@ def run_ours(args, rank, world, local_rank):
     warm = None
     if not args.no_warm and not slab_mode and args.state == "dark":
         ww = wl.synthetic_warm_state(w)
-        a.set_fields(*[t.contiguous() for t in ww.fields()])
+        wf = [t.contiguous() for t in ww.fields()]
         del ww
-        torch.cuda.empty_cache()
+        a.set_fields(*wf)
         warm_steps = min(args.steps, args.warm_steps)
-        warm = timed_leg(a, do_step, w.dt, warm_steps, args.warmup, world, stream, None)
+        warm = timed_leg(a, do_step, w.dt, warm_steps, args.warmup, world, stream, None,
+                         rewind=lambda: a.set_fields(*wf))
+        del wf
+        torch.cuda.empty_cache()
         warm["steps"] = warm_steps
     a.close()
     if rank != 0:
