@@ -277,22 +277,25 @@ step_v5_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
 #pragma unroll
                 for (int v = 0; v < 4; v++) { Wp[p][v] = u.v[p][v] + F[v]; Wm[p][v] = u.v[p][v] - F[v]; }
             }
-            f2 eWp[4], eWm[4];
-            {   // the x halo cell of the edge lanes (all lanes run it; only q = 0 / 31 use the result)
-                f2 e[4], ea, es, F[4];
+            float xw[4];
+            {   // the x halo cell of the edge lanes (all lanes run it; only q = 0 / 31 use the result): (U + F_x) of the
+                // cell left of the row for lane 0, (U - F_x) of the cell right of it for lane 31
+                float e[4], ea, es;
 #pragma unroll
-                for (int v = 0; v < 4; v++) e[v] = splat(buf[v * C::RS + mxh]);
-                closure2(e[0], e[1], e[2], e[3], ea, es);
-                flux_row(0, e, ea, es, F);
+                for (int v = 0; v < 4; v++) e[v] = buf[v * C::RS + mxh];
+                closure1(e[0], e[1], e[2], e[3], ea, es);
+                const float tt = es * e[1];
+                const float F[4] = {e[1], fmaf(tt, e[1], ea), tt * e[2], tt * e[3]};
+                const float sg = edge_r ? -1.0f : 1.0f;
 #pragma unroll
-                for (int v = 0; v < 4; v++) { eWp[v] = e[v] + F[v]; eWm[v] = e[v] - F[v]; }
+                for (int v = 0; v < 4; v++) xw[v] = fmaf(F[v], sg, e[v]);
             }
 #pragma unroll
             for (int v = 0; v < 4; v++) {
                 float left = __shfl_up_sync(0xffffffffu, hi(Wp[1][v]), 1);
                 float right = __shfl_down_sync(0xffffffffu, lo(Wm[0][v]), 1);
-                left = slct(left, lo(eWp[v]), q - 1);         // q == 0: the halo cell
-                right = slct(right, lo(eWm[v]), 30 - q);      // q == 31: the halo cell
+                left = slct(left, xw[v], q - 1);              // q == 0: the halo cell
+                right = slct(right, xw[v], 30 - q);           // q == 31: the halo cell
                 const f2 sx0 = pk(left + hi(Wm[0][v]), lo(Wp[0][v]) + lo(Wm[1][v]));
                 const f2 sx1 = pk(hi(Wp[0][v]) + hi(Wm[1][v]), lo(Wp[1][v]) + right);
                 t.v[0][v] = fma2(sx0, c.h, t.v[0][v]);

@@ -19,8 +19,9 @@ TOL_1STEP = float(os.environ.get("ATON_TOL_1STEP", "1e-4"))     # the north_star
 assert TOL_1STEP <= 1e-4
 TOL_L1 = 1e-3
 TOL_XVOL = 1e-3
-# None = the library's default = the product kernel (variant 4) on every grid it can tile (all cases below but the
-# ragged 40^3 one, which the default runs through the variant-2 fallback); 0 and 2 are the cross-check kernels
+# None = the library's default: the product kernel (variant 5, step_v5_kernel) on the 128-wide grids, its bit-identical
+# predecessor (variant 4) on the 32- and 64-wide ones, the variant-2 fallback on the ragged 40^3 one; 0 and 2 are the
+# cross-check kernels
 VARIANTS = [None, 0, 2]
 VIDS = ["default", "v0", "v2"]
 
@@ -49,9 +50,10 @@ def _cases():
         "cfg1_32": (lambda: wl.make_config(1), 60, 500),           # config 1 itself, its full 500 steps
         "cfg2_twin64": (lambda: twin(2, 64, 120), 60, 120),
         "cfg3_twin64": (lambda: twin(3, 64, 100), 50, 100),
-        "cfg3_twin40": (lambda: twin(3, 40, 100), 50, 100),       # 40: not tileable by variant 4 -> fallback kernel, ragged tail
+        "cfg3_twin40": (lambda: twin(3, 40, 100), 50, 100),       # 40: tileable by neither 5 nor 4 -> variant-2 fallback, ragged tail
         "cfg4_twin64": (lambda: twin(4, 64, 100), 50, 100),       # case A + clumping + coll. ion.
         "cfg5_twin32": (lambda: twin(5, 32, 80), 40, 80),
+        "cfg4_twin128": (lambda: twin(4, 128, 60), 30, 60),       # 128^3: the default is the product kernel, 16 rows per CTA
     }
 
 
@@ -102,13 +104,15 @@ def test_isothermal_and_no_collisions_switches(orc, variant):
                dict(cooling=1, coll_ion=0, redshift=9.0),
                # paper-form clumping (Eq.15): C_R = K nH^0.7 and C_I = K' nH^0.2
                dict(cooling=1, coll_ion=1, recomb_case=0, clump_model=2, clump_a=300.0, clump_b=0.7, clump_i_a=8.0, clump_i_b=0.2)):
-        w = twin(3, 32, 60)                  # 32^3: the default runs the product kernel
-        w.params.update(kw)
-        ww = _warm(orc, w, 40)
-        st, p = oracle_run(orc, ww, 1)
-        g, _ = gpu_run(ww, 1, variant)
-        err = max_rel_errors(g, st, p.c)
-        assert max(err.values()) <= TOL_1STEP, (kw, err)
+        # 32^3 (default: variant 4) for every kernel; 128^3 (default: the product kernel, every FLAGS instantiation of it)
+        for n, k in ((32, 40),) + (((128, 16),) if variant is None else ()):
+            w = twin(3, n, 60)
+            w.params.update(kw)
+            ww = _warm(orc, w, k)
+            st, p = oracle_run(orc, ww, 1)
+            g, _ = gpu_run(ww, 1, variant)
+            err = max_rel_errors(g, st, p.c)
+            assert max(err.values()) <= TOL_1STEP, (n, kw, err)
 
 
 @pytest.mark.parametrize("case", ["cfg1_32", "cfg3_twin64", "cfg4_twin64", "cfg3_twin40"])
@@ -270,9 +274,9 @@ def test_tiled_vs_reference_kernel():
 
 @pytest.mark.parametrize("variant", [2, 4], ids=["v2", "v4"])
 def test_fixup_path_statistics(variant):
-    """Cells that need sub-cycling are redone (variant 4: by the producing warp; variant 2: by the fix-up kernel),
-    counted, and nothing is left queued (a second identical context gives the same counts); an isothermal run never
-    sub-cycles (variant 4 still redoes its one source cell per step)."""
+    """Cells that need sub-cycling are redone by the fix-up kernel, counted, and nothing is left queued (a second
+    identical context gives the same counts); an isothermal run never sub-cycles (variant 4 still hands its one source
+    cell per step to the fix-up kernel)."""
     w = wl.make_config(1)
     g, d = gpu_run(w, 40, variant)
     assert d["cells_subcycled"] > 0 and d["subcycles_max"] > 1
@@ -368,8 +372,9 @@ def test_empty_sources_and_vacuum_conservation():
 
 
 # ------------------------------------------------------------------------------------------------
-# Non-cubic grids for the product kernel: x extents of one to eight 32-cell warp tiles (ragged last CTA), several y
-# tiles, ragged z chunks, sources on tile corners / edges and across every periodic seam.
+# Non-cubic grids for the tiled kernels (variant 5: 128-cell row segments, 8 or 16 rows per CTA; variant 4: x extents of
+# one to eight 32-cell warp tiles, ragged last CTA): several y tiles, ragged z chunks, sources on tile corners / edges and
+# across every periodic seam.
 # ------------------------------------------------------------------------------------------------
 def _slab_case(nx, ny, nz, flags7, seed, paper_clumping=False):
     """Random log-normal-ish density on an (nz, ny, nx) grid, sources on tile corners / edges, physics of
@@ -649,7 +654,7 @@ def _full_run(orc, w, steps):
 
 
 def test_config2_full_run_against_oracle(orc):
-    """Config 2 in full: its 128^3 grid, all of its 1000 steps, default kernel (variant 4), against the oracle run on
+    """Config 2 in full: its 128^3 grid, all of its 1000 steps, default kernel (variant 5), against the oracle run on
     the whole grid (about 100 s of oracle on 16 cores) -- BASELINE.json's full-run metric."""
     w = wl.make_config(2)
     assert w.n == 128 and w.n_steps == 1000
