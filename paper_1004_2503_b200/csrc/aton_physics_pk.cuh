@@ -27,13 +27,27 @@ __device__ __forceinline__ void closure2(f2 N, f2 gx, f2 gy, f2 gz, f2 &a, f2 &s
 
 // The same closure on ONE cell, operation for operation what closure2 does on each half (bit-identical): the x halo cell of
 // a row segment is a single cell, and a scalar MUFU / FMUL costs half the pipe time of the packed form on a splat pair.
+// Written with the _rn intrinsics so that every rounding is the one stated (none of closure2's operations is a bare
+// product followed by an add, so nothing in it is contracted on either path).
 __device__ __forceinline__ void closure1(float N, float gx, float gy, float gz, float &a, float &s) {
     const float inv = N > N_TINY ? m_rcp(N) : 0.0f;
-    const float rx = gx * inv, ry = gy * inv, rz = gz * inv;
-    const float ff = fminf(fmaf(rx, rx, fmaf(ry, ry, rz * rz)), 1.0f);
-    const float w = m_sqrt(fmaf(ff, -3.0f, 4.0f));
-    a = (w - 1.0f) * (N * (1.0f / 3.0f));
-    s = (inv * 3.0f) * m_rcp(w + 2.0f);
+    const float rx = __fmul_rn(gx, inv), ry = __fmul_rn(gy, inv), rz = __fmul_rn(gz, inv);
+    const float ff = fminf(__fmaf_rn(rx, rx, __fmaf_rn(ry, ry, __fmul_rn(rz, rz))), 1.0f);
+    const float w = m_sqrt(__fmaf_rn(ff, -3.0f, 4.0f));
+    a = __fmul_rn(__fsub_rn(w, 1.0f), __fmul_rn(N, 1.0f / 3.0f));
+    s = __fmul_rn(__fmul_rn(inv, 3.0f), m_rcp(__fadd_rn(w, 2.0f)));
+}
+// (U + sg F_x) of one cell, sg = +-1, with the roundings of the packed path as ptxas builds it: for the components
+// whose flux is a bare product (F_Gy = t G_y, F_Gz = t G_z) it contracts mul.rn.f32x2 + add.rn.f32x2 of
+// "u +- flux_row(0, ...)" into one FFMA2 (checked in SASS and bit for bit on 2^24 random cells), so U + sg t G is ONE
+// fma here too; F_Gx = fma(t, G_x, a) is already an fma and is added with its own rounding.
+__device__ __forceinline__ void xterm1(const float e[4], float a, float s, float sg, float w[4]) {
+    const float t = __fmul_rn(s, e[1]);
+    const float ts = __fmul_rn(t, sg);                       // exact
+    w[0] = __fmaf_rn(e[1], sg, e[0]);
+    w[1] = __fmaf_rn(__fmaf_rn(t, e[1], a), sg, e[1]);
+    w[2] = __fmaf_rn(ts, e[2], e[2]);
+    w[3] = __fmaf_rn(ts, e[3], e[3]);
 }
 
 // ---------------------------------------------------------------- rates on a pair (reading S7)

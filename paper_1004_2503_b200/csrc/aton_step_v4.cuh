@@ -324,11 +324,7 @@ step_v4_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
 #pragma unroll
                 for (int v = 0; v < 4; v++) e[v] = buf[v * C::RAW_FIELD + mxh];
                 closure1(e[0], e[1], e[2], e[3], ea, es);
-                const float tt = es * e[1];
-                const float F[4] = {e[1], fmaf(tt, e[1], ea), tt * e[2], tt * e[3]};
-                const float sg = edge_r ? -1.0f : 1.0f;
-#pragma unroll
-                for (int v = 0; v < 4; v++) xw[v] = fmaf(F[v], sg, e[v]);
+                xterm1(e, ea, es, edge_r ? -1.0f : 1.0f, xw);
             }
 #pragma unroll
             for (int v = 0; v < 4; v++) {
