@@ -5,6 +5,7 @@
 #include "aton_ctx.cuh"
 #include "aton_reduce.cuh"
 #include "aton_step_fused.cuh"
+#include "aton_step_hll.cuh"
 #include "aton_step_v4.cuh"
 #include "aton_step_v5.cuh"
 
@@ -147,7 +148,10 @@ template <int FLAGS>
 cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     const StepConst &sc = ctx->sc;
     const StepConstD &scd = ctx->scd;
-    if (ctx->p.flux == 1) {        // HLL intercell flux: one-thread-per-cell kernel, whatever the variant
+    // HLL intercell flux: the tiled kernel where a kernel variant 4 / 5 context's grid allows it (nx % 32 == 0,
+    // ny % 8 == 0; it shares their second half: mask, fix-up, fp64), else one thread per cell with the chemistry in place
+    const bool hll_tiled = ctx->p.flux == 1 && !ctx->slab && step_kernel_of(ctx) >= 4 && hll_tiled_grid_ok(ctx->g);
+    if (ctx->p.flux == 1 && !hll_tiled) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
         time_mark(ctx);
@@ -172,7 +176,9 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     ctx->fast_subcycles += (long long)ctx->plane * (ze - zb);
     cudaError_t e;
     time_mark(ctx);
-    if (kern == 5)
+    if (hll_tiled)
+        e = launch_step_hll_tiled<FLAGS>(f, ctx->g, sc, ctx->stream);
+    else if (kern == 5)
         e = launch_step_v5<FLAGS>(f, ctx->g, sc, v5_pick_w(ctx->g, ctx->tile_y), ctx->tile_z, ctx->stream, zb, ze);
     else if (kern == 4)
         e = launch_step_v4<FLAGS>(f, ctx->g, sc, wxq4, ctx->variant == 4 ? ctx->tile_z : 0, ctx->stream, zb, ze);

@@ -141,6 +141,29 @@ def test_hll_flux_against_oracle(orc, case):
     assert np.abs(g0["N"] - g["N"]).sum() > 1e-2 * np.abs(g["N"]).sum()
 
 
+def test_hll_tiled_kernel_agrees_with_the_one_thread_per_cell_kernel():
+    """The tiled HLL kernel (default on grids with nx % 32 == 0 and ny % 8 == 0: every cell closed once per plane, records
+    shared through shared memory, the product path's chemistry: fast sub-step + fix-up kernels) against step_hll_kernel
+    (variant 0: one thread per cell, chemistry in place) -- on grids whose tiles wrap every periodic seam, ragged z chunks
+    and nz = 1 included.  Same face formula in the same order: equal to rounding (both are held to the oracle separately,
+    test_hll_flux_against_oracle)."""
+    for shape, steps in (((64, 16, 37), 20), ((32, 8, 1), 6), ((96, 24, 5), 12)):
+        nx, ny, nz = shape
+        nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, True, seed=nx + nz)
+        p = dict(p, flux=1)
+        tiled, dt_ = _run_slab(5, (0, 0), nH, x, T, p, dx, pos, rate, steps)
+        ref, dr = _run_slab(0, (0, 0), nH, x, T, p, dx, pos, rate, steps)
+        assert dt_["n_nonfinite"] == 0 and dt_["photons_total"] > 0
+        for k in ("N", "Fx", "Fy", "Fz", "x", "T"):
+            num = np.abs(ref[k].astype(np.float64) - tiled[k]).sum()
+            den = np.abs(ref[k].astype(np.float64)).sum()
+            assert num <= 1e-5 * den, (shape, k, num / den)
+        for k in ("x", "T"):
+            assert np.allclose(ref[k], tiled[k], rtol=3e-4, atol=0), (shape, k)
+        assert dt_["subcycles_total"] == pytest.approx(dr["subcycles_total"], rel=1e-2)
+        assert dt_["photons_total"] == pytest.approx(dr["photons_total"], rel=1e-5)
+
+
 @pytest.mark.parametrize("variant", VARIANTS, ids=VIDS)
 def test_reduce_matches_oracle(orc, variant):
     w = wl.synthetic_warm_state(twin(4, 32, 10))
