@@ -296,6 +296,8 @@ def run_ours(args, rank, world, local_rank):
         a, do_step = sl.ctx, sl.step
     else:
         w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
+        if args.flux == "hll":          # the paper's other intercell flux; not the headline
+            w.params["flux"] = 1
         if args.state == "warm":
             w = wl.synthetic_warm_state(w)
         a = aton.from_workload(w)
@@ -373,6 +375,8 @@ def run_ours(args, rank, world, local_rank):
     if kvar == 4 and not (n % 32 == 0):
         kvar = 2
     kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel", 5: "step_v5_kernel"}[kvar]
+    if args.flux == "hll":
+        kname = "step_hll_tiled_kernel" if (kvar >= 4 and n % 32 == 0 and not slab_mode) else "step_hll_kernel"
     roofline = roofline_of(leg, cells, args.steps, peak, peak_src, recorded_traffic(n, "dark"), kname)
     if iso_ms:
         roofline["kernel_ms_isolated"] = iso_ms
@@ -403,6 +407,7 @@ def run_ours(args, rank, world, local_rank):
             "config": {"workload": f"config {cfg}: {n}^3 periodic box, lognormal density, {int(w.src_rate.numel())} sources, "
                                    f"physics flags {dict((k, w.params[k]) for k in ('recomb_case', 'cooling', 'coll_ion', 'clump_model'))}",
                        "state": args.state + f" start + {args.warmup} warm-up steps",
+                       "flux": "Lax-Friedrichs" if args.flux == "lf" else "HLL (not the headline flux)",
                        "l2": "working set per step (52 B/cell) exceeds the 126 MB L2" if 52 * cells > 4 * 126e6 else "fits in L2 (latency bound; not an HBM figure)",
                        "parallelism": (("z slabs of the one box (strong scaling)" if args.strong else "z slabs of one n x n x (n N) box")
                                        + ", halo planes exchanged every step inside the library, overlapped" if slab_mode
@@ -432,6 +437,7 @@ def main():
     ap.add_argument("--strong", action="store_true", help="--decomp slab: cut the config's own box N ways (strong scaling)")
     ap.add_argument("--no-warm", action="store_true", help="skip the second (synthetic warm state) leg")
     ap.add_argument("--warm-steps", type=int, default=50, help="timed steps of the warm leg (at most --steps)")
+    ap.add_argument("--flux", default="lf", choices=["lf", "hll"], help="intercell flux: Lax-Friedrichs (the headline) or HLL")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-isolated", action="store_true", help="skip the four single steps that time the step kernel alone")
     ap.add_argument("--no-cpu", action="store_true")
