@@ -376,7 +376,9 @@ def run_ours(args, rank, world, local_rank):
         kvar = 2
     kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel", 5: "step_v5_kernel"}[kvar]
     if args.flux == "hll":
-        kname = "step_hll_tiled_kernel" if (kvar >= 4 and n % 32 == 0 and not slab_mode) else "step_hll_kernel"
+        kname = "step_hll_kernel"
+        if kvar >= 4 and not slab_mode and n % 32 == 0:
+            kname = "step_hll_pk_kernel" if n % 64 == 0 else "step_hll_tiled_kernel"
     roofline = roofline_of(leg, cells, args.steps, peak, peak_src, recorded_traffic(n, "dark"), kname)
     if iso_ms:
         roofline["kernel_ms_isolated"] = iso_ms

@@ -6,6 +6,7 @@
 #include "aton_reduce.cuh"
 #include "aton_step_fused.cuh"
 #include "aton_step_hll.cuh"
+#include "aton_step_hll2.cuh"
 #include "aton_step_v4.cuh"
 #include "aton_step_v5.cuh"
 
@@ -176,8 +177,9 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     ctx->fast_subcycles += (long long)ctx->plane * (ze - zb);
     cudaError_t e;
     time_mark(ctx);
-    if (hll_tiled)
-        e = launch_step_hll_tiled<FLAGS>(f, ctx->g, sc, ctx->stream);
+    if (hll_tiled)      // two cells per thread on the packed forms where nx % 64 == 0, else one
+        e = hll_pk_grid_ok(ctx->g) ? launch_step_hll_pk<FLAGS>(f, ctx->g, sc, ctx->stream)
+                                   : launch_step_hll_tiled<FLAGS>(f, ctx->g, sc, ctx->stream);
     else if (kern == 5)
         e = launch_step_v5<FLAGS>(f, ctx->g, sc, v5_pick_w(ctx->g, ctx->tile_y), ctx->tile_z, ctx->stream, zb, ze);
     else if (kern == 4)
