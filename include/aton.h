@@ -65,7 +65,7 @@ typedef struct {
                             a <= 0 => C_I = 1 (the variant the paper also ran, L269-271) */
     int flux;            /* intercell flux ("HLL or the simpler Lax-Friedrich scheme"): 0 = Lax-Friedrichs at
                             speed c (the one the paper used; the product kernel); 1 = HLL with the M1 wave speeds (tiled
-                            kernels on grids with nx % 32 == 0 and ny % 8 == 0 -- packed fp32x2 where nx % 64 == 0: 2.3 x
+                            kernels on grids with nx % 32 == 0 and ny % 8 == 0 -- packed fp32x2 where nx % 64 == 0: 2.0 x
                             the Lax-Friedrichs step --, a one-thread-per-cell kernel on the others; undivided grids only) */
 } aton_params_t;
 

@@ -9,12 +9,18 @@
 //  * y faces: between own and the same pair of the row below / above (8-byte record reads); z faces from registers;
 //  * the tile's ring: the rows below / above as 32 pairs each (warps 0, 1), the cells left / right of each row as one odd
 //    pair per row (8 lanes of warp 2).
+//  * no plain global load in the loop (the lesson of variant 5, profiles/r02_d_step_v5.md): (N, G) of the next plane -- own
+//    pair and ring duty -- are staged by cp.async into thread-private double-buffered slots, x, T, n_H and the source word of
+//    the plane being finished into single ones; the records are double buffered by plane parity: one barrier per plane.
 // Same formulas as hll_cell / hll_speeds / hll_face (aton_step_ref.cuh); 1/(lambda+ - lambda-) by rcp.approx.
 #pragma once
 #include "aton_step_fused.cuh"
 
 namespace aton {
 
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+}
 __device__ __forceinline__ f2 fmax2(f2 a, f2 b) { return pk(fmaxf(lo(a), lo(b)), fmaxf(hi(a), hi(b))); }
 __device__ __forceinline__ f2 fmin2(f2 a, f2 b) { return pk(fminf(lo(a), lo(b)), fminf(hi(a), hi(b))); }
 
@@ -77,8 +83,11 @@ __device__ __forceinline__ void hll_face2(const HllPair &l, f2 lol, f2 hil, cons
     }
 }
 
+#ifndef HLLPK_DB
+#define HLLPK_DB 1       // 1: records double buffered by plane parity (one barrier per plane, 83 KB: 2 CTAs per SM); 0: two barriers
+#endif
 #ifndef HLLPK_MINB
-#define HLLPK_MINB 3     // 80 registers with 152 B of spills and 24 warps per SM: 3.72 against 3.84 ms per 512^3 step at 116 registers and 16
+#define HLLPK_MINB 2     // 116 registers, no spills, 16 warps per SM: 3.2 ms per 512^3 step (3 CTAs at 80 registers with single-buffered records: 4.4 ms)
 #endif
 struct HllPk {
     static constexpr int TXP = 32, TX = 2 * TXP, TY = 8, SY = TY + 2;
@@ -86,12 +95,20 @@ struct HllPk {
     static constexpr int NREC = 10;              // U0..U3, a, s, lo_x, hi_x, lo_y, hi_y
     static constexpr int PLANE = SY * RS;
     static constexpr int THREADS = TXP * TY;
+    static constexpr int NRING = 2 * TXP + TY;   // threads with a ring duty: the two ring rows (a pair each), one odd pair per tile row
+    static constexpr int NBUF = HLLPK_DB ? 2 : 1; // record buffers
+    static constexpr size_t SMEM = (size_t)NBUF * NREC * PLANE * sizeof(float)
+                                   + (size_t)(2 * 4 * THREADS + 2 * 4 * NRING + 4 * THREADS) * sizeof(float2);
 };
 
 template <int FLAGS>
 __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
     using C = HllPk;
-    __shared__ __align__(8) float rec[C::NREC][C::PLANE];
+    extern __shared__ __align__(16) float hsm[];
+    float (*rec)[C::NREC][C::PLANE] = reinterpret_cast<float (*)[C::NREC][C::PLANE]>(hsm);          // [NBUF]
+    float2 *stg = reinterpret_cast<float2 *>(hsm + C::NBUF * C::NREC * C::PLANE);                     // [2][4][THREADS]: own N, G of the next plane
+    float2 *rstg = stg + 2 * 4 * C::THREADS;                                                          // [2][4][NRING]: ring duty
+    float2 *xts = rstg + 2 * 4 * C::NRING;                                                            // [4][THREADS]: x, T, n_H, source word
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, z0 = blockIdx.z * lz;
     const int lzn = min(lz, g.nz - z0);
@@ -108,10 +125,34 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
     const int rcol_l = (y0 + tx) * g.nx + il, rcol_r = (y0 + tx) * g.nx + ir;   // (tx < TY only)
     const int rcol_slot = (tx + 1) * C::RS;                          // + 1: left cell, + TX + 2: right cell
 
-    auto put2 = [&](int r, int slot, f2 v) { *reinterpret_cast<float2 *>(&rec[r][slot]) = make_float2(lo(v), hi(v)); };
-    auto get2 = [&](int r, int slot) { const float2 v = *reinterpret_cast<const float2 *>(&rec[r][slot]); return pk(v.x, v.y); };
-    auto get11 = [&](int r, int slot) { return pk(rec[r][slot], rec[r][slot + 1]); };      // a pair at an odd column
-    auto load2 = [&](const float *p, int id) { const float2 v = __ldg(reinterpret_cast<const float2 *>(p + id)); return pk(v.x, v.y); };
+    const int rix = ty < 2 ? threadIdx.x : 2 * C::TXP + tx;          // ring duty index (ring_row / ring_col threads)
+    int par = 0;                                                    // record buffer of the plane being formed
+    auto put2 = [&](int r, int slot, f2 v) { *reinterpret_cast<float2 *>(&rec[par][r][slot]) = make_float2(lo(v), hi(v)); };
+    auto get2 = [&](int r, int slot) { const float2 v = *reinterpret_cast<const float2 *>(&rec[par][r][slot]); return pk(v.x, v.y); };
+    auto get11 = [&](int r, int slot) { return pk(rec[par][r][slot], rec[par][r][slot + 1]); };      // a pair at an odd column
+    auto sget = [&](const float2 *p) { const float2 v = *p; return pk(v.x, v.y); };
+    const float *src[4] = {f.N, f.Gx, f.Gy, f.Gz};
+    // stage plane kk into buffer b: the thread's own pair, and its ring duty if the plane belongs to the chunk
+    auto stage = [&](int b, int kk, bool inp) {
+        float2 *d = stg + (size_t)b * 4 * C::THREADS + threadIdx.x;
+        const int base = kk * plane;
+#pragma unroll
+        for (int v = 0; v < 4; v++) cp_async8(d + v * C::THREADS, src[v] + base + col);
+        if (inp) {
+            float2 *rd = rstg + (size_t)b * 4 * C::NRING + rix;
+            if (ring_row) {
+#pragma unroll
+                for (int v = 0; v < 4; v++) cp_async8(rd + v * C::NRING, src[v] + base + rrow_col);
+            } else if (ring_col) {
+#pragma unroll
+                for (int v = 0; v < 4; v++) {
+                    cp_async4(reinterpret_cast<float *>(rd + v * C::NRING), src[v] + base + rcol_l);
+                    cp_async4(reinterpret_cast<float *>(rd + v * C::NRING) + 1, src[v] + base + rcol_r);
+                }
+            }
+        }
+        cp_async_commit();
+    };
 
     const float mu = 2.0f * c.h;                                    // c dt / dx
     const f2 zero = splat(0.0f);
@@ -124,12 +165,36 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
     prev.a = zero; prev.s = zero;
     int idp = 0;
     int k = z0 == 0 ? g.nz - 1 : z0 - 1;
+    stage(0, k, false);
     for (int m = 0; m <= lzn + 1; m++) {
         const bool inpl = m >= 1 && m <= lzn;                       // plane m belongs to the chunk (CTA-uniform)
         const int id = k * plane + col;
+        const int kn = k + 1 == g.nz ? 0 : k + 1;
+        const int sb_ = m & 1;                                      // staging buffer of plane m
+        par = HLLPK_DB ? sb_ : 0;
+        cp_async_wait_all();                                        // this thread's part of plane m has landed
+        const float2 *sd = stg + (size_t)sb_ * 4 * C::THREADS + threadIdx.x;
         HllPair ce;
         HllSpeeds w;
-        hll_pair(load2(f.N, id), load2(f.Gx, id), load2(f.Gy, id), load2(f.Gz, id), ce, w);
+        hll_pair(sget(sd), sget(sd + C::THREADS), sget(sd + 2 * C::THREADS), sget(sd + 3 * C::THREADS), ce, w);
+        HllPair rc;                                                 // ring duty of plane m (read before the slots are re-staged)
+        HllSpeeds rw;
+        if (inpl && (ring_row || ring_col)) {
+            const float2 *rd = rstg + (size_t)sb_ * 4 * C::NRING + rix;
+            hll_pair(sget(rd), sget(rd + C::NRING), sget(rd + 2 * C::NRING), sget(rd + 3 * C::NRING), rc, rw);
+        }
+        // x, T, n_H and the source word of plane m-1 (finished at the end of this iteration), then the next plane's staging
+        const bool fin = m >= 2;
+        if (fin) {
+            float2 *xd = xts + threadIdx.x;
+            cp_async8(xd, f.x + idp);
+            cp_async8(xd + C::THREADS, f.T + idp);
+            cp_async8(xd + 2 * C::THREADS, f.nH + idp);
+            cp_async4(reinterpret_cast<float *>(xd + 3 * C::THREADS), f.src_bits + ((unsigned)idp >> 5));
+            cp_async_commit();
+        }
+        const bool more = m <= lzn;
+        if (more) stage(sb_ ^ 1, kn, m + 1 <= lzn);
         f2 Un[4] = {ce.U[0], ce.U[1], ce.U[2], ce.U[3]};
         if (inpl) {
             // ---- publish the records of the tile and of its ring
@@ -138,29 +203,21 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
             put2(4, own, ce.a); put2(5, own, ce.s);
             put2(6, own, w.lo[0]); put2(7, own, w.hi[0]); put2(8, own, w.lo[1]); put2(9, own, w.hi[1]);
             if (ring_row) {
-                const int rid = k * plane + rrow_col;
-                HllPair rc;
-                HllSpeeds rw;
-                hll_pair(load2(f.N, rid), load2(f.Gx, rid), load2(f.Gy, rid), load2(f.Gz, rid), rc, rw);
 #pragma unroll
                 for (int v = 0; v < 4; v++) put2(v, rrow_slot, rc.U[v]);
                 put2(4, rrow_slot, rc.a); put2(5, rrow_slot, rc.s);
                 put2(8, rrow_slot, rw.lo[1]); put2(9, rrow_slot, rw.hi[1]);
             } else if (ring_col) {
-                const int idl = k * plane + rcol_l, idr = k * plane + rcol_r;
-                HllPair rc;
-                HllSpeeds rw;
-                hll_pair(pk(__ldg(f.N + idl), __ldg(f.N + idr)), pk(__ldg(f.Gx + idl), __ldg(f.Gx + idr)),
-                         pk(__ldg(f.Gy + idl), __ldg(f.Gy + idr)), pk(__ldg(f.Gz + idl), __ldg(f.Gz + idr)), rc, rw);
                 const int sl = rcol_slot + 1, sr = rcol_slot + C::TX + 2;
 #pragma unroll
-                for (int v = 0; v < 4; v++) { rec[v][sl] = lo(rc.U[v]); rec[v][sr] = hi(rc.U[v]); }
-                rec[4][sl] = lo(rc.a); rec[4][sr] = hi(rc.a);
-                rec[5][sl] = lo(rc.s); rec[5][sr] = hi(rc.s);
-                rec[6][sl] = lo(rw.lo[0]); rec[6][sr] = hi(rw.lo[0]);
-                rec[7][sl] = lo(rw.hi[0]); rec[7][sr] = hi(rw.hi[0]);
+                for (int v = 0; v < 4; v++) { rec[par][v][sl] = lo(rc.U[v]); rec[par][v][sr] = hi(rc.U[v]); }
+                rec[par][4][sl] = lo(rc.a); rec[par][4][sr] = hi(rc.a);
+                rec[par][5][sl] = lo(rc.s); rec[par][5][sr] = hi(rc.s);
+                rec[par][6][sl] = lo(rw.lo[0]); rec[par][6][sr] = hi(rw.lo[0]);
+                rec[par][7][sl] = lo(rw.hi[0]); rec[par][7][sr] = hi(rw.hi[0]);
             }
-            __syncthreads();
+            __syncthreads();      // (with double-buffered records the one barrier of the plane: buffer `par` is not written again
+                                  // before every warp has passed the barrier of plane m+1)
             // ---- x: Fa between the pair shifted left by a cell and own, Fb between own and the pair shifted right
             {
                 HllPair nb;
@@ -195,14 +252,18 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
         if (m >= 1) {
             f2 Fz[4];                                               // the face between planes m-1 and m
             hll_face2<2>(prev, ploz, phiz, ce, w.lo[2], w.hi[2], Fz);
-            if (m >= 2) {                                           // plane m-1 is complete: chemistry, store
+            if (fin) {                                              // plane m-1 is complete: chemistry, store
 #pragma unroll
                 for (int v = 0; v < 4; v++) Unp[v] = Unp[v] - (Fz[v] - Fzb[v]) * mu;
                 // one straight-line chemistry sub-step; a source cell, or a cell that needs sub-cycling, keeps its transported
                 // values and is flagged for step_fixup_kernel / step_stiff_kernel, as in variants 4 and 5
-                const unsigned sb = (__ldg(f.src_bits + ((unsigned)idp >> 5)) >> (idp & 31)) & 3u;
-                f2 x2 = load2(f.x, idp), T2 = load2(f.T, idp);
-                const unsigned d = chem_fast2<FLAGS>(Unp[0], Unp[1], Unp[2], Unp[3], x2, T2, load2(f.nH, idp), c, sb);
+                if (more) cp_async_wait_1(); else cp_async_wait_all();     // the next plane's staging may still fly
+                const float2 *xd = xts + threadIdx.x;
+                f2 x2 = sget(xd), T2 = sget(xd + C::THREADS);
+                const f2 h2 = sget(xd + 2 * C::THREADS);
+                const unsigned sw = *reinterpret_cast<const unsigned *>(xd + 3 * C::THREADS);
+                const unsigned sb = (sw >> (idp & 31)) & 3u;
+                const unsigned d = chem_fast2<FLAGS>(Unp[0], Unp[1], Unp[2], Unp[3], x2, T2, h2, c, sb);
 #define ATON_ST2(ptr, A) *reinterpret_cast<float2 *>(ptr + idp) = make_float2(lo(A), hi(A))
                 ATON_ST2(f.N1, Unp[0]); ATON_ST2(f.Gx1, Unp[1]); ATON_ST2(f.Gy1, Unp[2]); ATON_ST2(f.Gz1, Unp[3]);
                 ATON_ST2(f.x, x2); ATON_ST2(f.T, T2);
@@ -216,8 +277,10 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
 #pragma unroll
         for (int v = 0; v < 4; v++) Unp[v] = Un[v];
         idp = id;
-        k = k + 1 == g.nz ? 0 : k + 1;
+        k = kn;
+#if !HLLPK_DB
         if (inpl) __syncthreads();                                  // the records are overwritten by the next plane
+#endif
     }
 }
 
@@ -230,7 +293,9 @@ cudaError_t launch_step_hll_pk(const FieldsIO &f, const Grid &g, const StepConst
     while (lz > 4 && tiles_xy * ((g.nz + lz - 1) / lz) < 4L * 4 * 148) lz >>= 1;
     lz = lz < g.nz ? lz : g.nz;
     const dim3 grid(g.nx / HllPk::TX, g.ny / HllPk::TY, (g.nz + lz - 1) / lz);
-    step_hll_pk_kernel<FLAGS><<<grid, HllPk::THREADS, 0, stream>>>(f, g, c, lz);
+    cudaError_t e = cudaFuncSetAttribute(step_hll_pk_kernel<FLAGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HllPk::SMEM);
+    if (e != cudaSuccess) return e;
+    step_hll_pk_kernel<FLAGS><<<grid, HllPk::THREADS, HllPk::SMEM, stream>>>(f, g, c, lz);
     return cudaGetLastError();
 }
 
