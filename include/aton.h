@@ -66,7 +66,7 @@ typedef struct {
     int flux;            /* intercell flux ("HLL or the simpler Lax-Friedrich scheme"): 0 = Lax-Friedrichs at
                             speed c (the one the paper used; the product kernel); 1 = HLL with the M1 wave speeds (tiled
                             kernels on grids with nx % 32 == 0 and ny % 8 == 0 -- packed fp32x2 where nx % 64 == 0: 2.0 x
-                            the Lax-Friedrichs step --, a one-thread-per-cell kernel on the others; undivided grids only) */
+                            the Lax-Friedrichs step --, a one-thread-per-cell kernel on the others; a slab context takes the tiled kernels only) */
 } aton_params_t;
 
 /* Global diagnostics (PAPER.md:L149 volume-weighted x, L303-305 mass-weighted, Eq.15 Gamma = c sigma_n N). */

@@ -151,8 +151,9 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     const StepConstD &scd = ctx->scd;
     // HLL intercell flux: the tiled kernel where a kernel variant 4 / 5 context's grid allows it (nx % 32 == 0,
     // ny % 8 == 0; it shares their second half: mask, fix-up, fp64), else one thread per cell with the chemistry in place
-    const bool hll_tiled = ctx->p.flux == 1 && !ctx->slab && step_kernel_of(ctx) >= 4 && hll_tiled_grid_ok(ctx->g);
+    const bool hll_tiled = ctx->p.flux == 1 && step_kernel_of(ctx) >= 4 && hll_tiled_grid_ok(ctx->g);
     if (ctx->p.flux == 1 && !hll_tiled) {
+        if (ctx->slab) return cudaErrorNotSupported;          // checked with a message in aton_init_slab
         const int threads = 256;
         const unsigned blocks = (unsigned)((ctx->nalloc + threads - 1) / threads);
         time_mark(ctx);
@@ -178,8 +179,8 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     cudaError_t e;
     time_mark(ctx);
     if (hll_tiled)      // two cells per thread on the packed forms where nx % 64 == 0, else one
-        e = hll_pk_grid_ok(ctx->g) ? launch_step_hll_pk<FLAGS>(f, ctx->g, sc, ctx->stream)
-                                   : launch_step_hll_tiled<FLAGS>(f, ctx->g, sc, ctx->stream);
+        e = hll_pk_grid_ok(ctx->g) ? launch_step_hll_pk<FLAGS>(f, ctx->g, sc, ctx->stream, zb, ze)
+                                   : launch_step_hll_tiled<FLAGS>(f, ctx->g, sc, ctx->stream, zb, ze);
     else if (kern == 5)
         e = launch_step_v5<FLAGS>(f, ctx->g, sc, v5_pick_w(ctx->g, ctx->tile_y), ctx->tile_z, ctx->stream, zb, ze);
     else if (kern == 4)
@@ -336,8 +337,8 @@ static int init_common(aton_t **out, const aton_grid_t *grid, const aton_box_t *
     if (params->clump_model < 0 || params->clump_model > 2 || params->c_cm_s < 0.0 || params->eps_sub < 0.0 ||
         params->max_sub < 0 || params->flux < 0 || params->flux > 1)
         return fail(nullptr, ATON_EINVAL, "aton_init: bad clump_model / c / eps_sub / max_sub / flux");
-    if (slab && params->flux != 0)
-        return fail(nullptr, ATON_EINVAL, "aton_init_slab: the HLL flux runs on undivided grids only");
+    if (slab && params->flux != 0 && !(grid->nx % 32 == 0 && grid->ny % 8 == 0))
+        return fail(nullptr, ATON_EINVAL, "aton_init_slab: the HLL flux on a slab needs nx %% 32 == 0 and ny %% 8 == 0 (the tiled kernels)");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();

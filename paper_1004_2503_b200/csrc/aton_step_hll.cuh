@@ -43,12 +43,12 @@ struct HllTile {
 };
 
 template <int FLAGS>
-__global__ void __launch_bounds__(HllTile::THREADS) step_hll_tiled_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
+__global__ void __launch_bounds__(HllTile::THREADS) step_hll_tiled_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     using C = HllTile;
     __shared__ float rec[C::NREC][C::NC];     // U0..U3, a, s, lo_x, hi_x, lo_y, hi_y of the tile and its ring, current plane
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, z0 = blockIdx.z * lz;
-    const int lzn = min(lz, g.nz - z0);
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, z0 = zb + blockIdx.z * lz;
+    const int lzn = min(lz, ze - z0);      // planes [zb, ze): the periodic grid, or a slab's own planes between its ghost planes
     const int plane = g.nx * g.ny;
     const int own = (ty + 1) * C::SX + tx + 1;                      // this thread's cell in the record frame
     const int col = (y0 + ty) * g.nx + x0 + tx;                     // ... inside a plane
@@ -151,13 +151,14 @@ __global__ void __launch_bounds__(HllTile::THREADS) step_hll_tiled_kernel(Fields
 inline bool hll_tiled_grid_ok(const Grid &g) { return g.nx % HllTile::TX == 0 && g.ny % HllTile::TY == 0; }
 
 template <int FLAGS>
-cudaError_t launch_step_hll_tiled(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream) {
+cudaError_t launch_step_hll_tiled(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream, int zb, int ze) {
+    const int nzr = ze - zb;
     const long tiles_xy = (long)(g.nx / HllTile::TX) * (g.ny / HllTile::TY);
     int lz = 32;      // largest power of two <= 32 that still gives >= 4 waves of 8 CTAs per SM
-    while (lz > 4 && tiles_xy * ((g.nz + lz - 1) / lz) < 4L * 8 * 148) lz >>= 1;
-    lz = lz < g.nz ? lz : g.nz;
-    const dim3 grid(g.nx / HllTile::TX, g.ny / HllTile::TY, (g.nz + lz - 1) / lz);
-    step_hll_tiled_kernel<FLAGS><<<grid, HllTile::THREADS, 0, stream>>>(f, g, c, lz);
+    while (lz > 4 && tiles_xy * ((nzr + lz - 1) / lz) < 4L * 8 * 148) lz >>= 1;
+    lz = lz < nzr ? lz : nzr;
+    const dim3 grid(g.nx / HllTile::TX, g.ny / HllTile::TY, (nzr + lz - 1) / lz);
+    step_hll_tiled_kernel<FLAGS><<<grid, HllTile::THREADS, 0, stream>>>(f, g, c, lz, zb, ze);
     return cudaGetLastError();
 }
 

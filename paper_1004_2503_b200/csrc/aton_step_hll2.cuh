@@ -102,7 +102,7 @@ struct HllPk {
 };
 
 template <int FLAGS>
-__global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel(FieldsIO f, Grid g, StepConst c, int lz) {
+__global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel(FieldsIO f, Grid g, StepConst c, int lz, int zb, int ze) {
     using C = HllPk;
     extern __shared__ __align__(16) float hsm[];
     float (*rec)[C::NREC][C::PLANE] = reinterpret_cast<float (*)[C::NREC][C::PLANE]>(hsm);          // [NBUF]
@@ -110,8 +110,8 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
     float2 *rstg = stg + 2 * 4 * C::THREADS;                                                          // [2][4][NRING]: ring duty
     float2 *xts = rstg + 2 * 4 * C::NRING;                                                            // [4][THREADS]: x, T, n_H, source word
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, z0 = blockIdx.z * lz;
-    const int lzn = min(lz, g.nz - z0);
+    const int x0 = blockIdx.x * C::TX, y0 = blockIdx.y * C::TY, z0 = zb + blockIdx.z * lz;
+    const int lzn = min(lz, ze - z0);      // planes [zb, ze): the periodic grid, or a slab's own planes between its ghost planes
     const int plane = g.nx * g.ny;
     const int own = (ty + 1) * C::RS + 2 + 2 * tx;                  // the pair's lo cell in the record frame (even: 8-byte aligned)
     const int col = (y0 + ty) * g.nx + x0 + 2 * tx;                 // ... inside a plane
@@ -287,15 +287,16 @@ __global__ void __launch_bounds__(HllPk::THREADS, HLLPK_MINB) step_hll_pk_kernel
 inline bool hll_pk_grid_ok(const Grid &g) { return g.nx % HllPk::TX == 0 && g.ny % HllPk::TY == 0; }
 
 template <int FLAGS>
-cudaError_t launch_step_hll_pk(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream) {
+cudaError_t launch_step_hll_pk(const FieldsIO &f, const Grid &g, const StepConst &c, cudaStream_t stream, int zb, int ze) {
+    const int nzr = ze - zb;
     const long tiles_xy = (long)(g.nx / HllPk::TX) * (g.ny / HllPk::TY);
     int lz = 32;      // largest power of two <= 32 that still gives >= 4 waves of 4 CTAs per SM
-    while (lz > 4 && tiles_xy * ((g.nz + lz - 1) / lz) < 4L * 4 * 148) lz >>= 1;
-    lz = lz < g.nz ? lz : g.nz;
-    const dim3 grid(g.nx / HllPk::TX, g.ny / HllPk::TY, (g.nz + lz - 1) / lz);
+    while (lz > 4 && tiles_xy * ((nzr + lz - 1) / lz) < 4L * 4 * 148) lz >>= 1;
+    lz = lz < nzr ? lz : nzr;
+    const dim3 grid(g.nx / HllPk::TX, g.ny / HllPk::TY, (nzr + lz - 1) / lz);
     cudaError_t e = cudaFuncSetAttribute(step_hll_pk_kernel<FLAGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HllPk::SMEM);
     if (e != cudaSuccess) return e;
-    step_hll_pk_kernel<FLAGS><<<grid, HllPk::THREADS, HllPk::SMEM, stream>>>(f, g, c, lz);
+    step_hll_pk_kernel<FLAGS><<<grid, HllPk::THREADS, HllPk::SMEM, stream>>>(f, g, c, lz, zb, ze);
     return cudaGetLastError();
 }
 

@@ -83,11 +83,15 @@ def _case(nx, ny, nz, seed=2):
 @pytest.mark.gpu
 # 128-wide grids run the product kernel (variant 5: 16 or 8 rows per CTA), the others the variant-4 fallback
 @pytest.mark.parametrize("shape,world", [((64, 8, 12), 2), ((32, 12, 13), 3), ((64, 8, 5), 5), ((32, 8, 9), 1),
-                                         ((128, 16, 12), 2), ((128, 8, 10), 3), ((256, 32, 7), 2)])
+                                         ((128, 16, 12), 2), ((128, 8, 10), 3), ((256, 32, 7), 2),
+                                         # the HLL flux on slabs: the packed tiled kernel (nx % 64 == 0) and the scalar one
+                                         ((64, 8, 12, "hll"), 2), ((32, 16, 9, "hll"), 3), ((128, 16, 7, "hll"), 2)])
 def test_slabs_on_one_gpu_equal_the_undivided_run(shape, world):
     from paper_1004_2503_b200 import aton
-    nx, ny, nz = shape
+    nx, ny, nz = shape[:3]
     nH, p, dx, pos, rate = _case(nx, ny, nz)
+    if len(shape) > 3:
+        p = dict(p, flux=1)
     x0, T0 = torch.full_like(nH, 1e-3), torch.full_like(nH, 100.0)
     dt, steps = wl.courant_dt(dx), 14
     full = aton.Aton(nx, ny, nz, dx * nx, p)
@@ -171,7 +175,7 @@ def test_slab_class_world_size_1_and_errors():
         aton.Aton(24, 8, 6, dx * 24, p, slab=(0, 3))       # variant 4 needs nx % 32 == 0
     hp = dict(p); hp.update(flux=1)
     with pytest.raises(aton.AtonError):
-        aton.Aton(32, 8, 6, dx * 32, hp, slab=(0, 3))      # the HLL kernel runs on undivided grids only
+        aton.Aton(32, 12, 6, dx * 32, hp, slab=(0, 3))     # the HLL flux on a slab needs the tiled kernels: ny % 8 == 0
     with pytest.raises(aton.AtonError):
         aton.Aton(32, 8, 6, dx * 32, p, slab=(4, 3))       # planes outside the grid
     a = aton.Aton(32, 8, 6, dx * 32, p)
