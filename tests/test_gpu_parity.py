@@ -141,6 +141,42 @@ def test_hll_flux_against_oracle(orc, case):
     assert np.abs(g0["N"] - g["N"]).sum() > 1e-2 * np.abs(g["N"]).sum()
 
 
+@pytest.mark.parametrize("flux", [0, 1], ids=["lf", "hll"])
+def test_switching_kernels_between_steps_changes_nothing_beyond_rounding(flux):
+    """One context, the kernel changed between chunks of steps (5 -> 4 -> 2 -> 0 -> 5; with flux = 1: packed tiled ->
+    one thread per cell -> tiled): no stale mask bit, queue entry, captured graph or argument block survives a switch.
+    Compared with the same steps run by the default kernel alone (the variants agree to rounding)."""
+    from paper_1004_2503_b200 import aton
+    nx, ny, nz = 128, 16, 10
+    nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, True, seed=77)
+    p = dict(p, flux=flux)
+    dt = wl.courant_dt(dx)
+    f = [torch.from_numpy(np.ascontiguousarray(v, dtype=np.float32)).cuda() for v in (nH, x, T)]
+
+    def run(plan):
+        a = aton.Aton(nx, ny, nz, dx * nx, p)
+        a.set_fields(*f)
+        a.set_sources(torch.from_numpy(pos), torch.from_numpy(rate))
+        for variant, n in plan:
+            a.set_kernel(variant)
+            a.step(dt, n)
+        g = {k: v.numpy() for k, v in a.get_fields(device="cpu").items()}
+        d = a.reduce()
+        a.close()
+        return g, d
+
+    ref, dref = run([(5, 16)])
+    mix, dmix = run([(5, 3), (4, 2), (2, 4), (0, 3), (5, 4)])
+    assert dmix["steps_done"] == 16 and dmix["n_nonfinite"] == 0 and dref["cells_subcycled"] > 0
+    for k in ("N", "Fx", "Fy", "Fz", "x", "T"):
+        num = np.abs(ref[k].astype(np.float64) - mix[k]).sum()
+        assert num <= 1e-5 * np.abs(ref[k].astype(np.float64)).sum(), (flux, k)
+    for k in ("x", "T"):
+        assert np.allclose(ref[k], mix[k], rtol=3e-4, atol=0), (flux, k)
+    assert dmix["photons_total"] == pytest.approx(dref["photons_total"], rel=1e-5)
+    assert dmix["subcycles_total"] == pytest.approx(dref["subcycles_total"], rel=1e-2)
+
+
 def test_hll_tiled_kernel_agrees_with_the_one_thread_per_cell_kernel():
     """The tiled HLL kernel (default on grids with nx % 32 == 0 and ny % 8 == 0: every cell closed once per plane, records
     shared through shared memory, the product path's chemistry: fast sub-step + fix-up kernels) against step_hll_kernel
