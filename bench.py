@@ -278,6 +278,8 @@ def run_ours(args, rank, world, local_rank):
         from paper_1004_2503_b200 import slab
         if args.strong:
             w = wl.make_config(cfg, n=n, device="cuda")               # every rank builds the same seeded box ...
+            if args.flux == "hll":
+                w.params["flux"] = 1
             zb, nzl = slab.slab_range(n, world, rank)                  # ... and keeps its planes
             sl = slab.SlabAton(n, n, n, w.box_cm, w.params, rank, world, native=True)
             part = [t[zb:zb + nzl].contiguous() for t in w.fields()]
@@ -287,6 +289,8 @@ def run_ours(args, rank, world, local_rank):
             cells = float(n) * n * nzl
         else:
             w = wl.make_config(cfg, n=n, device="cuda", seed=wl.SEED_BASE + cfg + 1000 * rank)
+            if args.flux == "hll":
+                w.params["flux"] = 1
             sl = slab.SlabAton(n, n, n * world, w.box_cm, w.params, rank, world, native=True)
             sl.set_fields(w.nH, w.x, w.T, w.N, w.Fx, w.Fy, w.Fz)
             pos = w.src_pos.clone()
@@ -377,7 +381,7 @@ def run_ours(args, rank, world, local_rank):
     kname = {0: "step_ref_kernel", 2: "step_fused_kernel", 4: "step_v4_kernel", 5: "step_v5_kernel"}[kvar]
     if args.flux == "hll":
         kname = "step_hll_kernel"
-        if kvar >= 4 and not slab_mode and n % 32 == 0:
+        if kvar >= 4 and n % 32 == 0:
             kname = "step_hll_pk_kernel" if n % 64 == 0 else "step_hll_tiled_kernel"
     roofline = roofline_of(leg, cells, args.steps, peak, peak_src, recorded_traffic(n, "dark"), kname)
     if iso_ms:
