@@ -1,7 +1,7 @@
 // C ABI of the ATON hot path (include/aton.h): context, uploads/downloads, source lists, the step
 // loop and the diagnostics.  The host only drives; every step of the path runs in
-// the kernels of aton_step_v4.cuh (product), aton_fixup.cuh, aton_step_fused.cuh / aton_step_ref.cuh
-// (fallback / cross-check) and aton_reduce.cuh.
+// the kernels of aton_step_v5.cuh (product), aton_step_v4.cuh / aton_step_fused.cuh (fallbacks for grids it cannot tile),
+// aton_fixup.cuh, aton_step_hll2.cuh / aton_step_hll.cuh (the HLL flux), aton_step_ref.cuh (cross-checks) and aton_reduce.cuh.
 #include "aton_ctx.cuh"
 #include "aton_reduce.cuh"
 #include "aton_step_fused.cuh"

@@ -61,9 +61,12 @@ __global__ void __launch_bounds__(128) step_stiff_kernel(const FixArgs *fa) {
 // shared-memory queue and processed one per thread once the queue holds a few hundred (or the scan ends),
 // so the data-dependent sub-cycle loops run on full warps.  Sources were injected by the step kernel.
 // ---------------------------------------------------------------------------------------------------
-constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS, FIXUP_GROUP = 8;
+constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRESH + 32 * FIXUP_THREADS;
+// FIXUP_GROUP chunks of FIXUP_THREADS words are scanned behind one vote: 8 on large grids (an empty scan of 1024^3 costs
+// 0.08 ms instead of 0.25), 2 or 1 on small ones so that the groups still outnumber the resident blocks (256^3 has 256
+// groups of 8: a block then redoes ~1300 cells, five batches per warp one after the other)
 
-template <int FLAGS>
+template <int FLAGS, int FIXUP_GROUP>
 __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
     __shared__ int queue[FIXUP_QCAP];
     __shared__ int qn, qhead;
@@ -179,19 +182,28 @@ __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixA
 }
 
 // cells [cell0, cell1) (whole planes; for the fallback grids the whole grid): mask words [cell0 / 32, ceil(cell1 / 32))
+template <int FLAGS, int GROUP>
+cudaError_t launch_step_fixup_g(const FixArgs *fa, int word0, int nwords, cudaStream_t stream) {
+    const int ngroups = (nwords + GROUP * FIXUP_THREADS - 1) / (GROUP * FIXUP_THREADS);
+    const int blocks = ngroups < 148 * 8 ? (ngroups > 0 ? ngroups : 1) : 148 * 8;
+    step_fixup_kernel<FLAGS, GROUP><<<blocks, FIXUP_THREADS, 0, stream>>>(fa, word0, nwords);
+    return cudaGetLastError();
+}
+
 template <int FLAGS>
 cudaError_t launch_step_fixup(const FixArgs *fa, long cell0, long cell1, cudaStream_t stream) {
     const int word0 = (int)(cell0 / 32), nwords = (int)((cell1 + 31) / 32) - word0;
-    const int ngroups = (nwords + FIXUP_GROUP * FIXUP_THREADS - 1) / (FIXUP_GROUP * FIXUP_THREADS);
-    const int blocks = ngroups < 148 * 8 ? (ngroups > 0 ? ngroups : 1) : 148 * 8;
-    step_fixup_kernel<FLAGS><<<blocks, FIXUP_THREADS, 0, stream>>>(fa, word0, nwords);
-    return cudaGetLastError();
+    const int chunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
+    if (chunks >= 8 * 148 * 8) return launch_step_fixup_g<FLAGS, 8>(fa, word0, nwords, stream);   // >= 512^3
+    if (chunks >= 2 * 148 * 8) return launch_step_fixup_g<FLAGS, 2>(fa, word0, nwords, stream);
+    return launch_step_fixup_g<FLAGS, 1>(fa, word0, nwords, stream);
 }
 
 template <int FLAGS>
 cudaError_t launch_step_stiff(const FixArgs *fa, cudaStream_t stream) {
     // wide enough that a few hundred thousand stiff cells get a thread each: the kernel then lasts as long as its
-    // slowest cell (tens of fp64 sub-cycles), not as long as a queue of them
+    // slowest cell (tens of fp64 sub-cycles), not as long as a queue of them.  (Fewer blocks on small grids change nothing:
+    // its 17 us floor with nothing queued is not the chain of per-block atomics.)
     step_stiff_kernel<FLAGS><<<148 * 8, 128, 0, stream>>>(fa);
     return cudaGetLastError();
 }
