@@ -194,9 +194,10 @@ cudaError_t launch_one(aton_ctx *ctx, const FieldsIO &f, int zb, int ze) {
     (void)scd;
     fix_mark(ctx);
     ctx->launches++;
-    e = launch_step_fixup<FLAGS>(ctx->fixargs + ctx->cur, (long)ctx->plane * zb, (long)ctx->plane * ze, ctx->stream);
+    const bool inline64 = (long)ctx->nalloc <= FIXUP_INLINE64_CELLS;      // small grid: the fp64 redo happens in the fix-up kernel
+    e = launch_step_fixup<FLAGS>(ctx->fixargs + ctx->cur, (long)ctx->plane * zb, (long)ctx->plane * ze, inline64, ctx->stream);
     fix_mark(ctx);
-    if (e == cudaSuccess && (FLAGS & F_COOL)) {       // without cooling nothing sub-cycles: no cell can be stiff
+    if (e == cudaSuccess && (FLAGS & F_COOL) && !inline64) {   // without cooling nothing sub-cycles: no cell can be stiff
         ctx->launches++;
         stiff_mark(ctx);
         e = launch_step_stiff<FLAGS>(ctx->fixargs + ctx->cur, ctx->stream);

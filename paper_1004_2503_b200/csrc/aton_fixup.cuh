@@ -66,14 +66,16 @@ constexpr int FIXUP_THREADS = 256, FIXUP_QTHRESH = 512, FIXUP_QCAP = FIXUP_QTHRE
 // 0.08 ms instead of 0.25), 2 or 1 on small ones so that the groups still outnumber the resident blocks (256^3 has 256
 // groups of 8: a block then redoes ~1300 cells, five batches per warp one after the other)
 
-template <int FLAGS, int FIXUP_GROUP>
-__global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
+// INLINE64: small grids (<= 2^21 cells) redo their stiff cells here, in place, instead of queueing them for step_stiff_kernel:
+// that kernel's launch and 17 us floor are a quarter of a 128^3 step
+template <int FLAGS, int FIXUP_GROUP, bool INLINE64>
+__global__ void __launch_bounds__(FIXUP_THREADS, INLINE64 ? 2 : 3) step_fixup_kernel(const FixArgs *fa, int word0, int nwords) {
     __shared__ int queue[FIXUP_QCAP];
     __shared__ int qn, qhead;
     const FieldsIO &f = fa->f;
     if (threadIdx.x == 0) { qn = 0; qhead = 0; }
     __syncthreads();
-    int nsub_extra = 0, nsub_max = 0, ncell = 0;
+    int nsub_extra = 0, nsub_max = 0, ncell = 0, n64 = 0;
     // redo the queued cells (all threads of the block call this together)
     auto drain = [&]() {
         const int n = qn;
@@ -97,6 +99,16 @@ __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixA
                 nsub_extra += ns - 1;
                 nsub_max = max(nsub_max, ns);
                 ncell++;
+            } else if (INLINE64) {          // stiff, small grid: the fp64 redo of step_stiff_kernel, here
+                double Nd = f.N1[id], gxd = f.Gx1[id], gyd = f.Gy1[id], gzd = f.Gz1[id], xd = f.x[id], Td = f.T[id];
+                if (f.fix_inject && ((__ldg(f.src_bits + ((unsigned)id >> 5)) >> (id & 31)) & 1u)) Nd += source_lookup_d(f, id, fa->cd.dt);
+                const int n64s = chemistry_f64<FLAGS>(Nd, gxd, gyd, gzd, xd, Td, (double)__ldg(f.nH + id), fa->cd);
+                f.N1[id] = (float)Nd; f.Gx1[id] = (float)gxd; f.Gy1[id] = (float)gyd; f.Gz1[id] = (float)gzd;
+                f.x[id] = (float)xd; f.T[id] = (float)Td;
+                nsub_extra += n64s - 1;
+                nsub_max = max(nsub_max, n64s);
+                ncell++;
+                n64++;
             } else {                        // stiff: the cell keeps its values; step_stiff_kernel redoes it in fp64
                 const unsigned slot = atomicAdd(f.stiff_n, 1u);
                 if (slot < f.stiff_cap) {
@@ -166,12 +178,14 @@ __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixA
     for (int o = 16; o > 0; o >>= 1) {
         nsub_extra += __shfl_xor_sync(0xffffffffu, nsub_extra, o);
         ncell += __shfl_xor_sync(0xffffffffu, ncell, o);
+        n64 += __shfl_xor_sync(0xffffffffu, n64, o);
         nsub_max = max(nsub_max, __shfl_xor_sync(0xffffffffu, nsub_max, o));
     }
     if ((threadIdx.x & 31) == 0 && ncell > 0) {
         atomicAdd(f.stats, (unsigned long long)nsub_extra);
         atomicMax(f.stats + 1, (unsigned long long)nsub_max);
         atomicAdd(f.stats + 2, (unsigned long long)ncell);
+        if (n64 > 0) atomicAdd(f.stats + 3, (unsigned long long)n64);
     }
     // the last block to finish re-arms the group cursor ([3] counts finished blocks)
     __syncthreads();
@@ -182,21 +196,25 @@ __global__ void __launch_bounds__(FIXUP_THREADS, 3) step_fixup_kernel(const FixA
 }
 
 // cells [cell0, cell1) (whole planes; for the fallback grids the whole grid): mask words [cell0 / 32, ceil(cell1 / 32))
-template <int FLAGS, int GROUP>
+template <int FLAGS, int GROUP, bool INLINE64>
 cudaError_t launch_step_fixup_g(const FixArgs *fa, int word0, int nwords, cudaStream_t stream) {
     const int ngroups = (nwords + GROUP * FIXUP_THREADS - 1) / (GROUP * FIXUP_THREADS);
     const int blocks = ngroups < 148 * 8 ? (ngroups > 0 ? ngroups : 1) : 148 * 8;
-    step_fixup_kernel<FLAGS, GROUP><<<blocks, FIXUP_THREADS, 0, stream>>>(fa, word0, nwords);
+    step_fixup_kernel<FLAGS, GROUP, INLINE64><<<blocks, FIXUP_THREADS, 0, stream>>>(fa, word0, nwords);
     return cudaGetLastError();
 }
 
+// grids of at most this many cells redo their stiff cells inside step_fixup_kernel (no step_stiff_kernel launch)
+constexpr long FIXUP_INLINE64_CELLS = 1L << 21;
+
 template <int FLAGS>
-cudaError_t launch_step_fixup(const FixArgs *fa, long cell0, long cell1, cudaStream_t stream) {
+cudaError_t launch_step_fixup(const FixArgs *fa, long cell0, long cell1, bool inline64, cudaStream_t stream) {
     const int word0 = (int)(cell0 / 32), nwords = (int)((cell1 + 31) / 32) - word0;
     const int chunks = (nwords + FIXUP_THREADS - 1) / FIXUP_THREADS;
-    if (chunks >= 8 * 148 * 8) return launch_step_fixup_g<FLAGS, 8>(fa, word0, nwords, stream);   // >= 512^3
-    if (chunks >= 2 * 148 * 8) return launch_step_fixup_g<FLAGS, 2>(fa, word0, nwords, stream);
-    return launch_step_fixup_g<FLAGS, 1>(fa, word0, nwords, stream);
+    if (inline64) return launch_step_fixup_g<FLAGS, 1, true>(fa, word0, nwords, stream);
+    if (chunks >= 8 * 148 * 8) return launch_step_fixup_g<FLAGS, 8, false>(fa, word0, nwords, stream);   // >= 512^3
+    if (chunks >= 2 * 148 * 8) return launch_step_fixup_g<FLAGS, 2, false>(fa, word0, nwords, stream);
+    return launch_step_fixup_g<FLAGS, 1, false>(fa, word0, nwords, stream);
 }
 
 template <int FLAGS>
