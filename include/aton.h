@@ -253,6 +253,24 @@ int aton_set_star_sources(aton_t *ctx, long long n, const float *pos, const doub
  * [H0 in 1/s, nH0 in cm^-3]; trapezoid rule.  Synchronises. */
 int aton_thomson_tau(aton_t *ctx, long long n, const double *z, const double *x, double nH0, double H0, double Om, double *tau);
 
+/* The raw sums of aton_reduce_sums for callers that must not allocate (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): no context, no cudaMalloc / cudaFree, no synchronisation -- two kernels enqueued on
+ * `cuda_stream` (a cudaStream_t cast to void*; NULL = the legacy default stream) of the CURRENT device.  The partial sums of
+ * the two-pass reduction live in a static __device__ array of 104 192 bytes that every GPU holds from the moment it loads the
+ * library until the process exits.
+ * nH, x, T, N, Fx, Fy, Fz: DEVICE arrays of `ncell` floats each (any grid shape), 16-byte aligned; c_cm_s <= 0 => 2.99792458e10.
+ * sums: DEVICE array of ATON_NOALLOC_NSUMS doubles, written when the stream reaches the call (the caller owns every array):
+ *   [0] cells [1] sum x [2] sum n_H x [3] sum n_H [4] sum N [5] sum n_H N [6] sum T [7] cells with x >= 0.5
+ *   [8] non-finite cells [9] max f = |F|/(cN) [10] min N [11] min n_H
+ * ([0]-[8] are entries [0]-[8] of aton_reduce_sums, [9] its [11], [10] its [13]; Eq.15).
+ * Limits: ncell a positive multiple of 4, at most 2^31 - 4 = 2 147 483 644 cells (ATON_EINVAL beyond, message in
+ * aton_last_error(NULL)).  Every call on a device SHARES the static array, which keeps the last call's contents (nothing in it
+ * has to start at zero: the rows a call reads are the rows it wrote): calls on one stream are ordered and safe, calls that
+ * OVERLAP on the GPU (other streams, concurrently replayed graphs) race and give wrong sums. */
+#define ATON_NOALLOC_NSUMS 12
+int aton_field_sums_noalloc(const float *nH, const float *x, const float *T, const float *N, const float *Fx, const float *Fy,
+                            const float *Fz, long long ncell, double c_cm_s, void *cuda_stream, double *sums);
+
 void aton_free(aton_t *ctx);
 
 /* Message of the last failing call on ctx (ctx-owned), or of the last failing aton_init if ctx is

@@ -22,10 +22,11 @@ EXPORTS = ("aton_init", "aton_set_fields", "aton_set_sources", "aton_courant_dt"
            "aton_kernel_time", "aton_fixup_time", "aton_init_slab", "aton_halo_pack", "aton_halo_unpack", "aton_set_mean_density",
            "aton_reduce_sums", "aton_diag_from_sums", "aton_set_mean_from_sums", "aton_comm_unique_id", "aton_comm_init",
            "aton_step_slab", "aton_reduce_global", "aton_sync_mean_density", "aton_clumping_blocks", "aton_histogram2d",
-           "aton_set_star_sources", "aton_thomson_tau", "aton_free", "aton_last_error")
+           "aton_set_star_sources", "aton_thomson_tau", "aton_field_sums_noalloc", "aton_free", "aton_last_error")
 Q_NH, Q_X, Q_NEUTRAL, Q_T, Q_N, Q_GAMMA = range(6)
 COMM_ID_BYTES = 128
 NSUMS = 15
+NOALLOC_NSUMS = 12
 
 
 class Grid(C.Structure):
@@ -129,6 +130,8 @@ def load_library(path: Optional[str] = None):
     L.aton_set_star_sources.argtypes = [vp, C.c_longlong, fp, dp, dp, dp] + [C.c_double] * 6 + [C.c_int]
     L.aton_thomson_tau.restype = C.c_int
     L.aton_thomson_tau.argtypes = [vp, C.c_longlong, dp, dp, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]
+    L.aton_field_sums_noalloc.restype = C.c_int
+    L.aton_field_sums_noalloc.argtypes = [fp, fp, fp, fp, fp, fp, fp, C.c_longlong, C.c_double, vp, dp]
     L.aton_free.restype = None
     L.aton_free.argtypes = [vp]
     L.aton_last_error.restype = C.c_char_p
@@ -330,6 +333,25 @@ class Aton:
 
     def launch_count(self) -> int:
         return int(self._L.aton_launch_count(self._h))
+
+
+def field_sums_noalloc(nH, x, T, N, Fx, Fy, Fz, out, c_cm_s: float = 0.0, stream=None):
+    """aton_field_sums_noalloc: the raw sums of aton_reduce_sums of seven float32 CUDA tensors of equal size, written into
+    `out` (a float64 CUDA tensor of NOALLOC_NSUMS elements) when the stream reaches the call.  Allocates nothing and does
+    not synchronise; every call on a device shares one static scratch array (calls that overlap on the GPU race)."""
+    L = load_library()
+    n = nH.numel()
+    for t in (nH, x, T, N, Fx, Fy, Fz):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == n):
+            raise ValueError("field_sums_noalloc: contiguous float32 CUDA tensors of one size, please")
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= NOALLOC_NSUMS):
+        raise ValueError(f"field_sums_noalloc: `out` must be a float64 CUDA tensor of {NOALLOC_NSUMS} elements")
+    st = (stream or torch.cuda.current_stream()).cuda_stream
+    rc = L.aton_field_sums_noalloc(*[C.c_void_p(t.data_ptr()) for t in (nH, x, T, N, Fx, Fy, Fz)], n, float(c_cm_s),
+                                   C.c_void_p(st), C.c_void_p(out.data_ptr()))
+    if rc != OK:
+        raise AtonError(rc, L.aton_last_error(None).decode())
+    return out
 
 
 def comm_unique_id() -> bytes:
