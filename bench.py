@@ -400,10 +400,14 @@ def run_ours(args, rank, world, local_rank):
         v, secs, cores = oracle_sample(cfg, args.cpu_sample_n, args.cpu_sample_steps, 3)
         n1 = max(32, args.cpu_sample_n // 2)
         v1, secs1, _ = oracle_sample(cfg, n1, max(4, args.cpu_sample_steps // 4), 2, threads=1)
+        vw, secsw, _ = oracle_sample(2, 128, 20, 40)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                "sample": f"config {cfg} twin at {args.cpu_sample_n}^3 (same dx, density statistics, source density), "
                          f"{args.cpu_sample_steps} steps after 3 warm-up, fp64, gcc -O2 + OpenMP",
                "value_1thread": v1, "seconds_1thread": secs1,
+               "value_warm_cfg2": vw, "seconds_warm_cfg2": secsw,
+               "sample_warm_cfg2": "config 2 on its own 128^3 grid, 20 steps after 40 oracle steps of warm-up (fronts present, "
+                                   "sub-cycling live): BASELINE.md's CPU-baseline plan",
                "sample_1thread": f"the same twin at {n1}^3, {max(4, args.cpu_sample_steps // 4)} steps after 2 warm-up, one thread"}
     diag = leg["diag"]
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
