@@ -183,16 +183,20 @@ def test_hll_tiled_kernel_agrees_with_the_one_thread_per_cell_kernel():
     (variant 0: one thread per cell, chemistry in place) -- on grids whose tiles wrap every periodic seam, ragged z chunks
     and nz = 1 included.  Same face formula in the same order: equal to rounding (both are held to the oracle separately,
     test_hll_flux_against_oracle)."""
-    for shape, steps in (((64, 16, 37), 20), ((32, 8, 1), 6), ((96, 24, 5), 12)):
+    # 64-wide grids run the packed kernel (step_hll_pk_kernel), 32- and 96-wide ones the scalar tiled kernel
+    for shape, steps in (((64, 16, 37), 20), ((32, 8, 1), 6), ((96, 24, 5), 12), ((64, 8, 1), 6), ((128, 8, 2), 8), ((192, 16, 33), 10)):
         nx, ny, nz = shape
         nH, x, T, p, dx, pos, rate = _slab_case(nx, ny, nz, True, seed=nx + nz)
         p = dict(p, flux=1)
         tiled, dt_ = _run_slab(5, (0, 0), nH, x, T, p, dx, pos, rate, steps)
         ref, dr = _run_slab(0, (0, 0), nH, x, T, p, dx, pos, rate, steps)
         assert dt_["n_nonfinite"] == 0 and dt_["photons_total"] > 0
+        # F components against their natural scale c sum N (reading S16): with nz = 1 or 2 the z flux vanishes by symmetry
+        # and what is left of it in either kernel is rounding noise
+        cn = wl.C_CM_S * np.abs(ref["N"].astype(np.float64)).sum()
         for k in ("N", "Fx", "Fy", "Fz", "x", "T"):
             num = np.abs(ref[k].astype(np.float64) - tiled[k]).sum()
-            den = np.abs(ref[k].astype(np.float64)).sum()
+            den = cn if k[0] == "F" else np.abs(ref[k].astype(np.float64)).sum()
             assert num <= 1e-5 * den, (shape, k, num / den)
         for k in ("x", "T"):
             assert np.allclose(ref[k], tiled[k], rtol=3e-4, atol=0), (shape, k)
