@@ -732,3 +732,14 @@ def test_config3_full_run_against_oracle(orc):
     assert w.n == 256 and w.n_steps == 2000
     err, diag = _full_run(orc, w, w.n_steps)
     print("config 3, 2000 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
+
+
+@pytest.mark.skipif(os.environ.get("ATON_SLOW4", "") != "1", reason="512^3 on the whole grid is ~15 min of oracle: set ATON_SLOW4=1")
+def test_config4_first_steps_on_the_whole_grid_against_oracle(orc):
+    """Config 4 on its full 512^3 grid (case A + recombination radiation, collisional ionisation, cooling, C_R = max(1, 1 + 2 delta),
+    2e4 sources), the first 120 of its 1000 steps, the WHOLE grid against the oracle (opt-in; the result of the round's run is
+    recorded in DESIGN.md) -- the sub-cube tests see 5 x 24^3 cells of this grid, this one all 1.3e8."""
+    w = wl.make_config(4)
+    assert w.n == 512 and w.n_steps == 1000
+    err, diag = _full_run(orc, w, 120)
+    print("config 4, 120 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
