@@ -743,3 +743,12 @@ def test_config4_first_steps_on_the_whole_grid_against_oracle(orc):
     assert w.n == 512 and w.n_steps == 1000
     err, diag = _full_run(orc, w, 120)
     print("config 4, 120 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
+
+
+@pytest.mark.skipif(os.environ.get("ATON_SLOW4", "") != "1", reason="512^3 on the whole grid is ~10 min of oracle: set ATON_SLOW4=1")
+def test_config4_warm_state_on_the_whole_grid_against_oracle(orc):
+    """The same grid from workloads.synthetic_warm_state (fronts everywhere: 47 % of the cells sub-cycle in the first step, the
+    fix-up and fp64 kernels carry a large share of the work), 16 steps, the whole grid against the oracle (opt-in)."""
+    w = wl.synthetic_warm_state(wl.make_config(4))
+    err, diag = _full_run(orc, w, 16)
+    print("config 4 warm, 16 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
