@@ -752,3 +752,14 @@ def test_config4_warm_state_on_the_whole_grid_against_oracle(orc):
     w = wl.synthetic_warm_state(wl.make_config(4))
     err, diag = _full_run(orc, w, 16)
     print("config 4 warm, 16 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
+
+
+def test_config3_warm_state_on_the_whole_grid_against_oracle(orc):
+    """Config 3's full 256^3 grid from workloads.synthetic_warm_state (fronts everywhere, about half of the cells sub-cycle in
+    the first step), 12 steps, every cell against the oracle: the fix-up / fp64 kernels under load at a config's real size,
+    in the default suite (about half a minute of oracle)."""
+    w = wl.synthetic_warm_state(wl.make_config(3))
+    assert w.n == 256
+    err, diag = _full_run(orc, w, 12)
+    assert diag["cells_subcycled"] > 10 * 256 ** 3 // 100 and diag["cells_fp64"] > 0
+    print("config 3 warm, 12 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
