@@ -763,3 +763,12 @@ def test_config3_warm_state_on_the_whole_grid_against_oracle(orc):
     err, diag = _full_run(orc, w, 12)
     assert diag["cells_subcycled"] > 10 * 256 ** 3 // 100 and diag["cells_fp64"] > 0
     print("config 3 warm, 12 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
+
+
+def test_config3_hll_flux_on_the_whole_grid_against_oracle(orc):
+    """The HLL flux (the packed tiled kernel, step_hll_pk_kernel, with several z chunks per column tile) on config 3's full
+    256^3 grid from the synthetic warm state, 8 steps, every cell against the oracle's orc_transport_hll."""
+    w = wl.synthetic_warm_state(wl.make_config(3))
+    w.params.update(flux=1)
+    err, diag = _full_run(orc, w, 8)
+    print("config 3 warm, HLL, 8 steps:", err, {k: diag[k] for k in ("x_vol", "cells_subcycled", "cells_fp64", "subcycles_max")})
